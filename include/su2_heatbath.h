@@ -1,0 +1,153 @@
+/*
+ * su2_heatbath.h — C ABI of the B200 (sm_100a) SU(2) pure-gauge heat-bath library.
+ *
+ * The library implements the data-parallel hot path of arxiv/paper_1104_5432
+ * ("Finite temperature lattice QCD with GPUs"): random SU(2) initialisation,
+ * checkerboarded heat-bath sweeps, the mean plaquette (§2.1) and the
+ * Polyakov loop (eq. 1). The paper prints no formula for the
+ * update; the readings [R1]..[R14] that define it are in DESIGN.md §3 (they restate
+ * SURVEY.md §8(c) and BASELINE.json north_star).
+ *
+ * General conventions
+ *  - Every call returns an int status: SU2_OK or one of the SU2_E* codes below.
+ *    No exception crosses the ABI, nothing calls exit().
+ *  - `su2_lattice*` is an opaque handle owned by the caller from create to destroy.
+ *    A handle is not thread-safe; different handles are independent. No global state.
+ *  - DEVICE pointers are marked [device], HOST pointers [host]. Out-pointers are
+ *    caller-owned.
+ *  - Lattice N_x x N_y x N_z x N_t, periodic, V sites; directions mu = 0,1,2,3 = x,y,z,t.
+ *    Site index s = x + N_x (y + N_y (z + N_z t)); parity p = (x+y+z+t) & 1.
+ *  - A link is a unit quaternion a = (a0,a1,a2,a3), U = a0 + i(a1 s1 + a2 s2 + a3 s3) [R1].
+ *  - Canonical HOST order of a configuration: [t][z][y][x][mu][4], i.e. element
+ *    ((s*4 + mu)*4 + c), real type = the lattice precision (float or double).
+ *  - DEVICE layout: 8 arrays indexed [p][mu], each V/2 quaternions,
+ *    element index h = s >> 1; array (p,mu) starts at quaternion (p*4+mu)*V/2.
+ *  - Work is enqueued on the handle's CUDA stream. Calls that return a value to the
+ *    host synchronise that stream; su2_heatbath_sweep and su2_init are asynchronous.
+ */
+#ifndef SU2_HEATBATH_H
+#define SU2_HEATBATH_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define SU2_API __attribute__((visibility("default")))
+#else
+#define SU2_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SU2_OK 0      /* success */
+#define SU2_EARG 1    /* bad argument (odd/too-small extent, bad precision/start, beta<=0 or
+                         non-finite, NULL pointer, wrong byte count) */
+#define SU2_EALLOC 2  /* device allocation failed */
+#define SU2_ECUDA 3   /* CUDA runtime error; sticky, message via su2_last_error */
+#define SU2_ESTATE 4  /* sweep or measurement before su2_init / su2_set_links */
+
+#define SU2_START_COLD 0
+#define SU2_START_HOT 1
+
+typedef struct su2_lattice su2_lattice;
+
+/* Bytes of device memory one configuration needs: 4*V quaternions of the precision.
+ * Returns 0 for invalid arguments. */
+SU2_API size_t su2_lattice_bytes(int Nx, int Ny, int Nz, int Nt, int precision);
+
+/* Create a lattice on the current CUDA device; the library allocates (cudaMalloc) the
+ * links and its reduction scratch and creates nothing else; work runs on the legacy
+ * default stream unless su2_set_stream is called.
+ *   precision: 32 (float4 links) or 64 (double links).
+ *   Each extent must be even and >= 2 (checkerboard + periodic wrap [R4]); V < 2^32
+ *   (the site index is one 32-bit Philox counter word [R5]).
+ * *out receives the handle. Errors: SU2_EARG, SU2_EALLOC, SU2_ECUDA. */
+SU2_API int su2_lattice_create(int Nx, int Ny, int Nz, int Nt, int precision, su2_lattice** out);
+
+/* As above, but the caller owns the link storage ("PyTorch owns memory"):
+ *   dev_links  [device] buffer of `bytes` >= su2_lattice_bytes(...), 32-byte aligned;
+ *              the library never frees it and it must outlive the handle.
+ *   cuda_stream a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream), may be 0.
+ * The small reduction scratch is still allocated by the library. */
+SU2_API int su2_lattice_create_external(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_links,
+                                size_t bytes, void* cuda_stream, su2_lattice** out);
+
+/* Free what the library allocated. NULL is a no-op (returns SU2_OK). */
+SU2_API int su2_lattice_destroy(su2_lattice* lat);
+
+/* Change the stream later work is enqueued on (cudaStream_t, may be 0). */
+SU2_API int su2_set_stream(su2_lattice* lat, void* cuda_stream);
+
+/* Row 1 of the path ("random SU(2) matrix initialization") [R9].
+ *   start = SU2_START_COLD: every link = (1,0,0,0).
+ *   start = SU2_START_HOT : Haar-random unit quaternion per link from
+ *           Philox4x32-10(counter = (s, 0, (1<<8)|(p<<2)|mu, 0), key = seed).
+ * Stores `seed` in the handle; it keys every later draw. Asynchronous. */
+SU2_API int su2_init(su2_lattice* lat, int start, uint64_t seed);
+
+/* Set the seed that keys later sweeps without touching the links (resume from a
+ * configuration loaded with su2_set_links). */
+SU2_API int su2_set_seed(su2_lattice* lat, uint64_t seed);
+
+/* Rows 2-6: one full heat-bath sweep = the 8 sub-steps (mu = 0..3 outer, parity 0,1
+ * inner) [R4]; each sub-step updates every U_mu(x) of that parity from its Wilson
+ * staple sum [R3] with a Kennedy-Pendleton draw [R6][R7], random numbers from
+ * Philox4x32-10(counter = (s, sweep_idx, (p<<2)|mu, n), key = seed) [R5].
+ * Same (links, seed, beta, sweep_idx) => same result on any launch geometry.
+ * The caller must not reuse a sweep_idx within a run. Asynchronous.
+ * Errors: SU2_EARG (beta <= 0 or not finite), SU2_ESTATE, SU2_ECUDA. */
+SU2_API int su2_heatbath_sweep(su2_lattice* lat, double beta, uint32_t sweep_idx);
+
+/* One sub-step (mu, parity) only — the unit the tests compare against the oracle. */
+SU2_API int su2_heatbath_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, int mu, int parity);
+
+/* Row 7: P = 1/(6V) sum_x sum_{mu<nu} 1/2 Tr U_mu(x) U_nu(x+mu) U_mu^dag(x+nu)
+ * U_nu^dag(x) [R10]; fp64 accumulation in a fixed order. Synchronises; *out [host] in [-1,1]. */
+SU2_API int su2_mean_plaquette(su2_lattice* lat, double* out);
+
+/* Row 8 (eq. 1): signed spatial average of
+ * 1/2 Tr prod_{t=0}^{N_t-1} U_t(x,t) [R11]. Synchronises; *out [host]. */
+SU2_API int su2_polyakov_loop(su2_lattice* lat, double* out);
+
+/* Rows 7+8 with one synchronisation: enqueue both reductions, then copy both doubles.
+ * Either out pointer may be NULL to skip that measurement. */
+SU2_API int su2_measure(su2_lattice* lat, double* plaquette_out, double* polyakov_out);
+
+/* Asynchronous form used for per-sweep measurement without a host round trip:
+ * enqueue the plaquette (slot 0) and Polyakov (slot 1) reductions of the current
+ * configuration and store the two doubles at dev_out[2*index], dev_out[2*index+1]
+ * ([device], caller-owned). No synchronisation. */
+SU2_API int su2_measure_async(su2_lattice* lat, double* dev_out, size_t index);
+
+/* NEXT-1 (eq. 3): on-axis Polyakov-loop correlator
+ * C(r) = < l(x) l(x + r e_i) >, averaged over all spatial x and the 3 spatial axes i,
+ * r = 1..rmax (rmax <= min spatial extent / 2), l(x) = 1/2 Tr L(x) (real in SU(2)).
+ * out [host] receives rmax doubles. Synchronises. */
+SU2_API int su2_polyakov_correlator(su2_lattice* lat, int rmax, double* out);
+
+/* Configuration I/O in canonical host order (see top). bytes must equal
+ * su2_lattice_bytes(...). Both synchronise. su2_set_links marks the lattice initialised.
+ * host pointers may be pageable or pinned. */
+SU2_API int su2_get_links(su2_lattice* lat, void* host_dst, size_t bytes);
+SU2_API int su2_set_links(su2_lattice* lat, const void* host_src, size_t bytes);
+
+/* Block until all work enqueued on the handle's stream has finished. */
+SU2_API int su2_synchronize(su2_lattice* lat);
+
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+SU2_API uint64_t su2_launch_count(const su2_lattice* lat);
+
+/* [device] pointer to the links in device layout (for callers that own the memory
+ * model; NULL on a NULL handle). */
+SU2_API void* su2_device_links(su2_lattice* lat);
+
+/* Message of the last error on this handle ("" if none); static string for a code. */
+SU2_API const char* su2_last_error(const su2_lattice* lat);
+SU2_API const char* su2_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SU2_HEATBATH_H */

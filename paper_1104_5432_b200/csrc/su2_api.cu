@@ -1,0 +1,329 @@
+// su2_api.cu — the C-ABI boundary (include/su2_heatbath.h): handle, argument
+// checking, error capture, stream plumbing. No arithmetic of the method lives here.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/su2_heatbath.h"
+#include "su2_launch.h"
+
+using namespace su2;
+
+struct su2_lattice {
+    Geom g;
+    int precision;
+    void* links;
+    bool owns_links;
+    cudaStream_t stream;
+    uint64_t seed;
+    bool initialised;
+    Scratch sc;
+    uint64_t launches;
+    int sticky;  // sticky error code
+    char msg[256];
+};
+
+static int fail(su2_lattice* lat, int code, const char* what, cudaError_t ce = cudaSuccess)
+{
+    if (lat) {
+        if (ce != cudaSuccess)
+            snprintf(lat->msg, sizeof lat->msg, "%s: %s", what, cudaGetErrorString(ce));
+        else
+            snprintf(lat->msg, sizeof lat->msg, "%s", what);
+        if (code == SU2_ECUDA) lat->sticky = code;
+    }
+    return code;
+}
+#define CK(lat, call)                                              \
+    do {                                                           \
+        cudaError_t ce__ = (call);                                 \
+        if (ce__ != cudaSuccess) return fail(lat, SU2_ECUDA, #call, ce__); \
+    } while (0)
+#define ENTER(lat)                       \
+    do {                                 \
+        if (!(lat)) return SU2_EARG;     \
+        if ((lat)->sticky) return (lat)->sticky; \
+    } while (0)
+
+static bool valid_dims(int Nx, int Ny, int Nz, int Nt, int precision)
+{
+    const int n[4] = {Nx, Ny, Nz, Nt};
+    uint64_t V = 1;
+    for (int d = 0; d < 4; ++d) {
+        if (n[d] < 2 || (n[d] & 1)) return false;
+        V *= (uint64_t)n[d];
+        if (V >= (1ull << 32)) return false;
+    }
+    return precision == 32 || precision == 64;
+}
+
+extern "C" size_t su2_lattice_bytes(int Nx, int Ny, int Nz, int Nt, int precision)
+{
+    if (!valid_dims(Nx, Ny, Nz, Nt, precision)) return 0;
+    return (size_t)Nx * Ny * Nz * Nt * 4 * 4 * (precision == 32 ? sizeof(float) : sizeof(double));
+}
+
+static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_links, size_t bytes, void* stream,
+                       bool external, su2_lattice** out)
+{
+    if (!out) return SU2_EARG;
+    *out = nullptr;
+    if (!valid_dims(Nx, Ny, Nz, Nt, precision)) return SU2_EARG;
+    const size_t need = su2_lattice_bytes(Nx, Ny, Nz, Nt, precision);
+    if (external && (!dev_links || bytes < need || ((uintptr_t)dev_links & 31))) return SU2_EARG;
+
+    su2_lattice* lat = new (std::nothrow) su2_lattice;
+    if (!lat) return SU2_EALLOC;
+    memset(lat, 0, sizeof *lat);
+    Geom& g = lat->g;
+    g.n[0] = Nx; g.n[1] = Ny; g.n[2] = Nz; g.n[3] = Nt;
+    g.nxh = Nx / 2;
+    g.sy = g.nxh;
+    g.sz = g.nxh * Ny;
+    g.st = g.nxh * Ny * Nz;
+    g.vh = (uint32_t)((uint64_t)Nx * Ny * Nz * Nt / 2);
+    g.nb[0] = g.nb[1] = g.nb[2] = g.nb[3] = 0;
+    if (tiled_ok(g)) {
+        g.nb[0] = g.nxh >> kTileLog2[0];
+        g.nb[1] = Ny >> kTileLog2[1];
+        g.nb[2] = Nz >> kTileLog2[2];
+        g.nb[3] = Nt >> kTileLog2[3];
+    }
+    lat->precision = precision;
+    lat->stream = (cudaStream_t)stream;
+    lat->owns_links = !external;
+    lat->links = dev_links;
+
+    cudaError_t ce = cudaSuccess;
+    if (!external) ce = cudaMalloc(&lat->links, need);
+    const uint64_t v3 = (uint64_t)Nx * Ny * Nz;
+    lat->sc.n_partials = partials_needed(g);
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.partials, lat->sc.n_partials * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.field, v3 * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.out, (2 + kMaxR) * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.err, sizeof(int));
+    if (ce == cudaSuccess) ce = cudaMemset(lat->sc.err, 0, sizeof(int));
+    if (ce != cudaSuccess) {
+        const int code = (ce == cudaErrorMemoryAllocation) ? SU2_EALLOC : SU2_ECUDA;
+        cudaGetLastError();
+        su2_lattice_destroy(lat);
+        return code;
+    }
+    *out = lat;
+    return SU2_OK;
+}
+
+extern "C" int su2_lattice_create(int Nx, int Ny, int Nz, int Nt, int precision, su2_lattice** out)
+{
+    return create_impl(Nx, Ny, Nz, Nt, precision, nullptr, 0, nullptr, false, out);
+}
+
+extern "C" int su2_lattice_create_external(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_links,
+                                           size_t bytes, void* cuda_stream, su2_lattice** out)
+{
+    return create_impl(Nx, Ny, Nz, Nt, precision, dev_links, bytes, cuda_stream, true, out);
+}
+
+extern "C" int su2_lattice_destroy(su2_lattice* lat)
+{
+    if (!lat) return SU2_OK;
+    if (lat->owns_links && lat->links) cudaFree(lat->links);
+    if (lat->sc.partials) cudaFree(lat->sc.partials);
+    if (lat->sc.field) cudaFree(lat->sc.field);
+    if (lat->sc.out) cudaFree(lat->sc.out);
+    if (lat->sc.err) cudaFree(lat->sc.err);
+    delete lat;
+    return SU2_OK;
+}
+
+extern "C" int su2_set_stream(su2_lattice* lat, void* cuda_stream)
+{
+    ENTER(lat);
+    lat->stream = (cudaStream_t)cuda_stream;
+    return SU2_OK;
+}
+
+extern "C" int su2_init(su2_lattice* lat, int start, uint64_t seed)
+{
+    ENTER(lat);
+    if (start != SU2_START_COLD && start != SU2_START_HOT) return fail(lat, SU2_EARG, "su2_init: bad start");
+    lat->launches += launch_init(lat->links, lat->g, lat->precision, start, seed, lat->stream);
+    CK(lat, cudaGetLastError());
+    lat->seed = seed;
+    lat->initialised = true;
+    return SU2_OK;
+}
+
+extern "C" int su2_set_seed(su2_lattice* lat, uint64_t seed)
+{
+    ENTER(lat);
+    lat->seed = seed;
+    return SU2_OK;
+}
+
+static int check_beta(su2_lattice* lat, double beta)
+{
+    if (!(beta > 0.0) || !isfinite(beta)) return fail(lat, SU2_EARG, "beta must be finite and > 0");
+    if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised (su2_init / su2_set_links)");
+    return SU2_OK;
+}
+
+extern "C" int su2_heatbath_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, int mu, int parity)
+{
+    ENTER(lat);
+    if (int rc = check_beta(lat, beta)) return rc;
+    if (mu < 0 || mu > 3 || (parity != 0 && parity != 1)) return fail(lat, SU2_EARG, "bad mu / parity");
+    lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, parity, beta, lat->seed,
+                                             sweep_idx, lat->sc.err, lat->stream);
+    CK(lat, cudaGetLastError());
+    return SU2_OK;
+}
+
+extern "C" int su2_heatbath_sweep(su2_lattice* lat, double beta, uint32_t sweep_idx)
+{
+    ENTER(lat);
+    if (int rc = check_beta(lat, beta)) return rc;
+    for (int mu = 0; mu < 4; ++mu)      // [R4] direction outer,
+        for (int p = 0; p < 2; ++p) {   //      parity inner
+            lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, p, beta, lat->seed,
+                                                     sweep_idx, lat->sc.err, lat->stream);
+        }
+    CK(lat, cudaGetLastError());
+    return SU2_OK;
+}
+
+// synchronise and surface device-side flags
+static int sync_and_check(su2_lattice* lat)
+{
+    int flags = 0;
+    CK(lat, cudaMemcpyAsync(&flags, lat->sc.err, sizeof(int), cudaMemcpyDeviceToHost, lat->stream));
+    CK(lat, cudaStreamSynchronize(lat->stream));
+    if (flags & 1) return fail(lat, SU2_ECUDA, "Kennedy-Pendleton trial cap (10000) hit: alpha = beta*k too small");
+    return SU2_OK;
+}
+
+extern "C" int su2_synchronize(su2_lattice* lat)
+{
+    ENTER(lat);
+    return sync_and_check(lat);
+}
+
+extern "C" int su2_measure_async(su2_lattice* lat, double* dev_out, size_t index)
+{
+    ENTER(lat);
+    if (!dev_out) return fail(lat, SU2_EARG, "su2_measure_async: NULL dev_out");
+    if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
+    lat->launches += launch_plaquette(lat->links, lat->g, lat->precision, lat->sc, dev_out + 2 * index, lat->stream);
+    lat->launches +=
+        launch_polyakov(lat->links, lat->g, lat->precision, lat->sc, dev_out + 2 * index + 1, lat->stream);
+    CK(lat, cudaGetLastError());
+    return SU2_OK;
+}
+
+extern "C" int su2_measure(su2_lattice* lat, double* plaquette_out, double* polyakov_out)
+{
+    ENTER(lat);
+    if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
+    if (plaquette_out)
+        lat->launches += launch_plaquette(lat->links, lat->g, lat->precision, lat->sc, lat->sc.out, lat->stream);
+    if (polyakov_out)
+        lat->launches += launch_polyakov(lat->links, lat->g, lat->precision, lat->sc, lat->sc.out + 1, lat->stream);
+    CK(lat, cudaGetLastError());
+    double host[2] = {0, 0};
+    CK(lat, cudaMemcpyAsync(host, lat->sc.out, sizeof host, cudaMemcpyDeviceToHost, lat->stream));
+    if (int rc = sync_and_check(lat)) return rc;
+    if (plaquette_out) *plaquette_out = host[0];
+    if (polyakov_out) *polyakov_out = host[1];
+    return SU2_OK;
+}
+
+extern "C" int su2_mean_plaquette(su2_lattice* lat, double* out)
+{
+    if (!out) return lat ? fail(lat, SU2_EARG, "NULL out") : SU2_EARG;
+    return su2_measure(lat, out, nullptr);
+}
+
+extern "C" int su2_polyakov_loop(su2_lattice* lat, double* out)
+{
+    if (!out) return lat ? fail(lat, SU2_EARG, "NULL out") : SU2_EARG;
+    return su2_measure(lat, nullptr, out);
+}
+
+extern "C" int su2_polyakov_correlator(su2_lattice* lat, int rmax, double* out)
+{
+    ENTER(lat);
+    if (!out) return fail(lat, SU2_EARG, "NULL out");
+    if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
+    int nmin = lat->g.n[0] < lat->g.n[1] ? lat->g.n[0] : lat->g.n[1];
+    if (lat->g.n[2] < nmin) nmin = lat->g.n[2];
+    if (rmax < 1 || rmax > nmin / 2 || rmax > kMaxR) return fail(lat, SU2_EARG, "rmax out of range");
+    lat->launches += launch_polyakov(lat->links, lat->g, lat->precision, lat->sc, lat->sc.out + 1, lat->stream);
+    lat->launches += launch_polyakov_correlator(lat->g, lat->sc, rmax, lat->sc.out + 2, lat->stream);
+    CK(lat, cudaGetLastError());
+    CK(lat, cudaMemcpyAsync(out, lat->sc.out + 2, rmax * sizeof(double), cudaMemcpyDeviceToHost, lat->stream));
+    return sync_and_check(lat);
+}
+
+extern "C" int su2_get_links(su2_lattice* lat, void* host_dst, size_t bytes)
+{
+    ENTER(lat);
+    const Geom& g = lat->g;
+    const size_t need = su2_lattice_bytes(g.n[0], g.n[1], g.n[2], g.n[3], lat->precision);
+    if (!host_dst || bytes != need) return fail(lat, SU2_EARG, "su2_get_links: bad buffer");
+    if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
+    void* stage = nullptr;
+    if (cudaMalloc(&stage, need) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(lat, SU2_EALLOC, "su2_get_links: staging buffer");
+    }
+    lat->launches += launch_to_canonical(lat->links, stage, g, lat->precision, lat->stream);
+    cudaError_t ce = cudaGetLastError();
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(host_dst, stage, need, cudaMemcpyDeviceToHost, lat->stream);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(lat->stream);
+    cudaFree(stage);
+    if (ce != cudaSuccess) return fail(lat, SU2_ECUDA, "su2_get_links", ce);
+    return SU2_OK;
+}
+
+extern "C" int su2_set_links(su2_lattice* lat, const void* host_src, size_t bytes)
+{
+    ENTER(lat);
+    const Geom& g = lat->g;
+    const size_t need = su2_lattice_bytes(g.n[0], g.n[1], g.n[2], g.n[3], lat->precision);
+    if (!host_src || bytes != need) return fail(lat, SU2_EARG, "su2_set_links: bad buffer");
+    void* stage = nullptr;
+    if (cudaMalloc(&stage, need) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(lat, SU2_EALLOC, "su2_set_links: staging buffer");
+    }
+    cudaError_t ce = cudaMemcpyAsync(stage, host_src, need, cudaMemcpyHostToDevice, lat->stream);
+    if (ce == cudaSuccess) {
+        lat->launches += launch_to_device_layout(stage, lat->links, g, lat->precision, lat->stream);
+        ce = cudaGetLastError();
+    }
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(lat->stream);
+    cudaFree(stage);
+    if (ce != cudaSuccess) return fail(lat, SU2_ECUDA, "su2_set_links", ce);
+    lat->initialised = true;
+    return SU2_OK;
+}
+
+extern "C" uint64_t su2_launch_count(const su2_lattice* lat) { return lat ? lat->launches : 0; }
+
+extern "C" void* su2_device_links(su2_lattice* lat) { return lat ? lat->links : nullptr; }
+
+extern "C" const char* su2_last_error(const su2_lattice* lat) { return lat ? lat->msg : "NULL handle"; }
+
+extern "C" const char* su2_strerror(int code)
+{
+    switch (code) {
+        case SU2_OK: return "ok";
+        case SU2_EARG: return "bad argument";
+        case SU2_EALLOC: return "device allocation failed";
+        case SU2_ECUDA: return "CUDA runtime error";
+        case SU2_ESTATE: return "bad state: lattice not initialised";
+        default: return "unknown error code";
+    }
+}

@@ -1,0 +1,179 @@
+// su2_device.cuh — device-side building blocks of the SU(2) heat-bath path (sm_100a).
+//
+// Written from DESIGN.md §3 (readings [R1]..[R14]); shares nothing with oracle/.
+//   [R1] quaternion algebra          [R5] Philox4x32-10 keying + uniform rules
+//   [R3] staple sum                  [R6] Kennedy-Pendleton draw
+//   [R7] direction + composition     [R9] Shoemake hot start
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace su2 {
+
+// ---------------------------------------------------------------- geometry
+// Device layout: array (p,mu) holds the V/2 links U_mu(x) of the
+// sites with parity p, element h = s>>1 = hx + nxh*(y + Ny*(z + Nz*t)), hx = x>>1.
+struct Geom {
+    int n[4];        // Nx, Ny, Nz, Nt
+    int nxh;         // Nx/2
+    int sy, sz, st;  // strides of y, z, t in half-index units: nxh, nxh*Ny, nxh*Ny*Nz
+    uint32_t vh;     // V/2
+    int nb[4];       // tiled launch: number of tiles along hx, y, z, t
+};
+
+// ---------------------------------------------------------------- quaternions
+template <typename Real>
+struct Quat {
+    Real a0, a1, a2, a3;
+};
+
+template <typename Real>
+struct LinkPtr;  // storage element type of one link
+template <>
+struct LinkPtr<float> {
+    typedef float4 type;
+};
+struct __align__(32) double4a {
+    double x, y, z, w;
+};
+template <>
+struct LinkPtr<double> {
+    typedef double4a type;
+};
+
+// Loads go through the non-coherent path: within one sub-step no array that is
+// read is written, and L1 is invalidated at every launch.
+__device__ __forceinline__ Quat<float> ldq(const float4* p)
+{
+    float4 v = __ldg(p);
+    return {v.x, v.y, v.z, v.w};
+}
+__device__ __forceinline__ Quat<double> ldq(const double4a* p)
+{
+    Quat<double> q;
+    // one 256-bit load per link (sm_100+)
+    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+                 : "=d"(q.a0), "=d"(q.a1), "=d"(q.a2), "=d"(q.a3)
+                 : "l"(p));
+    return q;
+}
+__device__ __forceinline__ void stq(float4* p, const Quat<float>& q)
+{
+    *p = make_float4(q.a0, q.a1, q.a2, q.a3);
+}
+__device__ __forceinline__ void stq(double4a* p, const Quat<double>& q)
+{
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(q.a0), "d"(q.a1), "d"(q.a2), "d"(q.a3)
+                 : "memory");
+}
+
+// [R1] c = op(a) * op(b), op = dagger when DA / DB:
+//   c0 = a0 b0 - a.b ; cvec = a0 b + b0 a - a x b ; dagger flips the vector part.
+template <bool DA, bool DB, typename Real>
+__device__ __forceinline__ Quat<Real> qmul(const Quat<Real>& a, const Quat<Real>& b)
+{
+    const Real a1 = DA ? -a.a1 : a.a1, a2 = DA ? -a.a2 : a.a2, a3 = DA ? -a.a3 : a.a3;
+    const Real b1 = DB ? -b.a1 : b.a1, b2 = DB ? -b.a2 : b.a2, b3 = DB ? -b.a3 : b.a3;
+    Quat<Real> c;
+    c.a0 = a.a0 * b.a0 - a1 * b1 - a2 * b2 - a3 * b3;
+    c.a1 = a.a0 * b1 + b.a0 * a1 - (a2 * b3 - a3 * b2);
+    c.a2 = a.a0 * b2 + b.a0 * a2 - (a3 * b1 - a1 * b3);
+    c.a3 = a.a0 * b3 + b.a0 * a3 - (a1 * b2 - a2 * b1);
+    return c;
+}
+// scalar part only of a * b^dagger  ( = 4-vector dot product )
+template <typename Real>
+__device__ __forceinline__ Real qdot(const Quat<Real>& a, const Quat<Real>& b)
+{
+    return a.a0 * b.a0 + a.a1 * b.a1 + a.a2 * b.a2 + a.a3 * b.a3;
+}
+
+// ---------------------------------------------------------------- Philox4x32-10 [R5]
+struct Words {
+    uint32_t w0, w1, w2, w3;
+};
+__device__ __forceinline__ Words philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                               uint32_t k1)
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        c0 = hi1 ^ c1 ^ k0;
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1;
+        c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    return {c0, c1, c2, c3};
+}
+// counter = (site, sweep_idx, (purpose<<8)|(parity<<2)|mu, call n), key = seed
+__device__ __forceinline__ Words draw(uint64_t seed, uint32_t s, uint32_t sweep, uint32_t tag, uint32_t n)
+{
+    return philox4x32_10(s, sweep, tag, n, (uint32_t)seed, (uint32_t)(seed >> 32));
+}
+
+// ---------------------------------------------------------------- per-precision math
+template <typename Real>
+struct M;
+template <>
+struct M<float> {
+    // fp32 rule: u = (2*(w>>9)+1) * 2^-24, exact, strictly inside (0,1)
+    static __device__ __forceinline__ float uniform(uint32_t w)
+    {
+        return (float)(2u * (w >> 9) + 1u) * (1.0f / 16777216.0f);
+    }
+    static __device__ __forceinline__ float log(float x) { return logf(x); }
+    static __device__ __forceinline__ float sqrt(float x) { return sqrtf(x); }
+    static __device__ __forceinline__ float rcp(float x) { return 1.0f / x; }
+    static __device__ __forceinline__ float cos2pi(float x) { return cospif(2.0f * x); }
+    static __device__ __forceinline__ void sincos2pi(float x, float* s, float* c) { sincospif(2.0f * x, s, c); }
+    static __device__ __forceinline__ float tiny() { return 1e-20f; }
+};
+template <>
+struct M<double> {
+    // fp64 rule: u = (w + 0.5) * 2^-32, exact
+    static __device__ __forceinline__ double uniform(uint32_t w)
+    {
+        return fma((double)w, 1.0 / 4294967296.0, 1.0 / 8589934592.0);
+    }
+    static __device__ __forceinline__ double log(double x) { return ::log(x); }
+    static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
+    static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
+    static __device__ __forceinline__ double cos2pi(double x) { return cospi(2.0 * x); }
+    static __device__ __forceinline__ void sincos2pi(double x, double* s, double* c) { sincospi(2.0 * x, s, c); }
+    static __device__ __forceinline__ double tiny() { return 1e-30; }
+};
+
+// [R9] Shoemake: uniform unit quaternion from three uniforms
+template <typename Real>
+__device__ __forceinline__ Quat<Real> haar_from_words(const Words& w)
+{
+    const Real u1 = M<Real>::uniform(w.w0), u2 = M<Real>::uniform(w.w1), u3 = M<Real>::uniform(w.w2);
+    const Real r1 = M<Real>::sqrt((Real)1 - u1), r2 = M<Real>::sqrt(u1);
+    Real s2, c2, s3, c3;
+    M<Real>::sincos2pi(u2, &s2, &c2);
+    M<Real>::sincos2pi(u3, &s3, &c3);
+    return {r1 * s2, r1 * c2, r2 * s3, r2 * c3};
+}
+
+// ---------------------------------------------------------------- block reduction
+// warp shuffle + fixed-order block tree in fp64; valid result in thread 0.
+// `red` must hold blockDim.x/32 doubles.
+__device__ __forceinline__ double block_sum(double v, double* red)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) red[wid] = v;
+    __syncthreads();
+    double tot = 0.0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < nw; ++i) tot += red[i];
+    __syncthreads();
+    return tot;
+}
+
+}  // namespace su2

@@ -1,0 +1,223 @@
+// su2_heatbath.cu — init and heat-bath sub-step kernels (rows 1-6 of SURVEY.md §8(a)).
+//
+// One thread updates one link U_mu(x) of the sub-step's parity:
+//   neighbour addressing (row 2) -> 18 vector loads + 12 quaternion products (row 3)
+//   -> k, alpha (row 4) -> Philox (row 5) -> Kennedy-Pendleton loop, compose, store (row 6).
+// Formulas: DESIGN.md §3 [R1]-[R9]. The paper's own kernels (texture vs global
+// memory) are prior art for GT200/Fermi; here link reads are
+// 128/256-bit non-coherent loads and the 2.4x neighbour reuse is served by L1
+// through a compact 4-D CTA tile.
+#include "su2_launch.h"
+
+namespace su2 {
+
+struct Site {
+    int hx, y, z, t;  // hx = x>>1
+};
+
+// half-index deltas of the 8 neighbours; r = low bit of x
+struct Nbr {
+    int up[4], dn[4];
+};
+__device__ __forceinline__ Nbr neighbours(const Geom& g, const Site& c, int r)
+{
+    Nbr d;
+    d.up[0] = r ? ((c.hx + 1 == g.nxh) ? -(g.nxh - 1) : 1) : 0;
+    d.dn[0] = r ? 0 : ((c.hx == 0) ? (g.nxh - 1) : -1);
+    d.up[1] = (c.y + 1 == g.n[1]) ? -(g.n[1] - 1) * g.sy : g.sy;
+    d.dn[1] = (c.y == 0) ? (g.n[1] - 1) * g.sy : -g.sy;
+    d.up[2] = (c.z + 1 == g.n[2]) ? -(g.n[2] - 1) * g.sz : g.sz;
+    d.dn[2] = (c.z == 0) ? (g.n[2] - 1) * g.sz : -g.sz;
+    d.up[3] = (c.t + 1 == g.n[3]) ? -(g.n[3] - 1) * g.st : g.st;
+    d.dn[3] = (c.t == 0) ? (g.n[3] - 1) * g.st : -g.st;
+    return d;
+}
+
+template <typename Real, int MU>
+__device__ __forceinline__ void heatbath_site(typename LinkPtr<Real>::type* __restrict__ links, const Geom& g,
+                                              int p, const Site& c, Real beta, uint64_t seed, uint32_t sweep,
+                                              int* __restrict__ err)
+{
+    typedef typename LinkPtr<Real>::type L;
+    const int r = (c.y + c.z + c.t + p) & 1;
+    const int h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
+    const Nbr d = neighbours(g, c, r);
+    const size_t vh = g.vh;
+    const L* same = links + (size_t)(p * 4) * vh;        // arrays of parity p
+    const L* oppo = links + (size_t)((1 - p) * 4) * vh;  // arrays of parity 1-p
+
+    // [R3] staple sum, nu ascending, forward then backward, products left to right
+    Quat<Real> v = {0, 0, 0, 0};
+#pragma unroll
+    for (int nu = 0; nu < 4; ++nu) {
+        if (nu == MU) continue;
+        const Quat<Real> a = ldq(oppo + nu * vh + (h + d.up[MU]));             // U_nu(x+mu)
+        const Quat<Real> b = ldq(oppo + MU * vh + (h + d.up[nu]));             // U_mu(x+nu)
+        const Quat<Real> cc = ldq(same + nu * vh + h);                         // U_nu(x)
+        const Quat<Real> a2 = ldq(same + nu * vh + (h + d.up[MU] + d.dn[nu]));  // U_nu(x+mu-nu)
+        const Quat<Real> b2 = ldq(oppo + MU * vh + (h + d.dn[nu]));            // U_mu(x-nu)
+        const Quat<Real> c2 = ldq(oppo + nu * vh + (h + d.dn[nu]));            // U_nu(x-nu)
+        const Quat<Real> f = qmul<false, true>(qmul<false, true>(a, b), cc);
+        const Quat<Real> w = qmul<false, false>(qmul<true, true>(a2, b2), c2);
+        v.a0 += f.a0; v.a1 += f.a1; v.a2 += f.a2; v.a3 += f.a3;
+        v.a0 += w.a0; v.a1 += w.a1; v.a2 += w.a2; v.a3 += w.a3;
+    }
+
+    // [R5] counter = (s, sweep, (p<<2)|mu, n)
+    const uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
+    const uint32_t tag = ((uint32_t)p << 2) | (uint32_t)MU;
+    const Words wd = draw(seed, s, sweep, tag, 0u);
+
+    const Real k2 = v.a0 * v.a0 + v.a1 * v.a1 + v.a2 * v.a2 + v.a3 * v.a3;
+    Quat<Real> u;
+    if (k2 < M<Real>::tiny()) {  // [R8]
+        u = haar_from_words<Real>(wd);
+    } else {
+        const Real alpha = beta * M<Real>::sqrt(k2);
+        const Real inv_alpha = M<Real>::rcp(alpha);
+        // [R6] Kennedy-Pendleton
+        Real delta = 0;
+        uint32_t n = 1;
+        for (;;) {
+            const Words w = draw(seed, s, sweep, tag, n);
+            const Real R = M<Real>::uniform(w.w0), Rp = M<Real>::uniform(w.w1);
+            const Real Rpp = M<Real>::uniform(w.w2), Rppp = M<Real>::uniform(w.w3);
+            const Real cs = M<Real>::cos2pi(Rp);
+            delta = -(M<Real>::log(R) + cs * cs * M<Real>::log(Rpp)) * inv_alpha;
+            if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) break;
+            if (++n > 10000u) {  // unreachable for alpha >~ 1e-4; flag, keep x0 = 1
+                atomicOr(err, 1);
+                delta = 0;
+                break;
+            }
+        }
+        // [R7] direction on the sphere of radius sqrt(delta(2-delta)), compose with Vbar^dagger
+        const Real x0 = (Real)1 - delta;
+        const Real rad = M<Real>::sqrt(fmax(delta * ((Real)2 - delta), (Real)0));
+        const Real cth = (Real)1 - (Real)2 * M<Real>::uniform(wd.w0);
+        const Real sth = M<Real>::sqrt(fmax((Real)1 - cth * cth, (Real)0));
+        Real sphi, cphi;
+        M<Real>::sincos2pi(M<Real>::uniform(wd.w1), &sphi, &cphi);
+        const Quat<Real> X = {x0, rad * sth * cphi, rad * sth * sphi, rad * cth};
+        u = qmul<false, true>(X, v);  // X * v^dagger = k * (X * Vbar^dagger); k drops out below
+    }
+    const Real inv = M<Real>::rcp(M<Real>::sqrt(u.a0 * u.a0 + u.a1 * u.a1 + u.a2 * u.a2 + u.a3 * u.a3));
+    u.a0 *= inv; u.a1 *= inv; u.a2 *= inv; u.a3 *= inv;
+    stq(links + (size_t)(p * 4 + MU) * vh + h, u);
+}
+
+// tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile
+template <typename Real, int MU, int LHX, int LY, int LZ, int LT>
+__global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT))
+    heatbath_tiled_kernel(typename LinkPtr<Real>::type* __restrict__ links, const Geom g, int p, Real beta,
+                          uint64_t seed, uint32_t sweep, int* __restrict__ err)
+{
+    int b = blockIdx.x;
+    const int bx = b % g.nb[0]; b /= g.nb[0];
+    const int by = b % g.nb[1]; b /= g.nb[1];
+    const int bz = b % g.nb[2];
+    const int bt = b / g.nb[2];
+    const int tid = threadIdx.x;
+    Site c;
+    c.hx = (bx << LHX) + (tid & ((1 << LHX) - 1));
+    c.y = (by << LY) + ((tid >> LHX) & ((1 << LY) - 1));
+    c.z = (bz << LZ) + ((tid >> (LHX + LY)) & ((1 << LZ) - 1));
+    c.t = (bt << LT) + (tid >> (LHX + LY + LZ));
+    heatbath_site<Real, MU>(links, g, p, c, beta, seed, sweep, err);
+}
+
+// linear launch: thread i <-> half-index h = i; any even extents
+template <typename Real, int MU>
+__global__ void __launch_bounds__(kBlock)
+    heatbath_linear_kernel(typename LinkPtr<Real>::type* __restrict__ links, const Geom g, int p, Real beta,
+                           uint64_t seed, uint32_t sweep, int* __restrict__ err)
+{
+    const uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
+    if (h >= g.vh) return;
+    Site c;
+    uint32_t q = h / (uint32_t)g.nxh;
+    c.hx = (int)(h - q * (uint32_t)g.nxh);
+    uint32_t q2 = q / (uint32_t)g.n[1];
+    c.y = (int)(q - q2 * (uint32_t)g.n[1]);
+    c.t = (int)(q2 / (uint32_t)g.n[2]);
+    c.z = (int)(q2 - (uint32_t)c.t * (uint32_t)g.n[2]);
+    heatbath_site<Real, MU>(links, g, p, c, beta, seed, sweep, err);
+}
+
+// [R9] init: one thread per link of the device layout
+template <typename Real>
+__global__ void __launch_bounds__(kBlock)
+    init_kernel(typename LinkPtr<Real>::type* __restrict__ links, const Geom g, int start, uint64_t seed)
+{
+    const uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
+    if (h >= g.vh) return;
+    const int arr = blockIdx.y;  // p*4 + mu
+    const int p = arr >> 2, mu = arr & 3;
+    Quat<Real> u = {1, 0, 0, 0};
+    if (start == 1) {
+        uint32_t q = h / (uint32_t)g.nxh;
+        uint32_t q2 = q / (uint32_t)g.n[1];
+        const uint32_t y = q - q2 * (uint32_t)g.n[1];
+        const uint32_t t = q2 / (uint32_t)g.n[2];
+        const uint32_t z = q2 - t * (uint32_t)g.n[2];
+        const uint32_t r = (y + z + t + (uint32_t)p) & 1u;
+        const uint32_t s = 2u * h + r;
+        const Words w = draw(seed, s, 0u, (1u << 8) | ((uint32_t)p << 2) | (uint32_t)mu, 0u);
+        u = haar_from_words<Real>(w);
+    }
+    stq(links + (size_t)arr * g.vh + h, u);
+}
+
+bool tiled_ok(const Geom& g)
+{
+    return g.nxh % (1 << kTileLog2[0]) == 0 && g.n[1] % (1 << kTileLog2[1]) == 0 &&
+           g.n[2] % (1 << kTileLog2[2]) == 0 && g.n[3] % (1 << kTileLog2[3]) == 0;
+}
+
+template <typename Real, int MU>
+static int launch_substep_t(void* links, const Geom& g, int parity, double beta, uint64_t seed, uint32_t sweep,
+                            int* err, cudaStream_t st)
+{
+    typedef typename LinkPtr<Real>::type L;
+    if (tiled_ok(g)) {
+        constexpr int T = 1 << (kTileLog2[0] + kTileLog2[1] + kTileLog2[2] + kTileLog2[3]);
+        const unsigned grid = (unsigned)(g.nb[0] * g.nb[1] * g.nb[2] * g.nb[3]);
+        heatbath_tiled_kernel<Real, MU, kTileLog2[0], kTileLog2[1], kTileLog2[2], kTileLog2[3]>
+            <<<grid, T, 0, st>>>((L*)links, g, parity, (Real)beta, seed, sweep, err);
+    } else {
+        const unsigned grid = (g.vh + kBlock - 1) / kBlock;
+        heatbath_linear_kernel<Real, MU><<<grid, kBlock, 0, st>>>((L*)links, g, parity, (Real)beta, seed, sweep, err);
+    }
+    return 1;
+}
+
+template <typename Real>
+static int launch_substep_p(void* links, const Geom& g, int mu, int parity, double beta, uint64_t seed,
+                            uint32_t sweep, int* err, cudaStream_t st)
+{
+    switch (mu) {
+        case 0: return launch_substep_t<Real, 0>(links, g, parity, beta, seed, sweep, err, st);
+        case 1: return launch_substep_t<Real, 1>(links, g, parity, beta, seed, sweep, err, st);
+        case 2: return launch_substep_t<Real, 2>(links, g, parity, beta, seed, sweep, err, st);
+        default: return launch_substep_t<Real, 3>(links, g, parity, beta, seed, sweep, err, st);
+    }
+}
+
+int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
+                            uint64_t seed, uint32_t sweep, int* err, cudaStream_t st)
+{
+    return precision == 32 ? launch_substep_p<float>(links, g, mu, parity, beta, seed, sweep, err, st)
+                           : launch_substep_p<double>(links, g, mu, parity, beta, seed, sweep, err, st);
+}
+
+int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st)
+{
+    const dim3 grid((g.vh + kBlock - 1) / kBlock, 8);
+    if (precision == 32)
+        init_kernel<float><<<grid, kBlock, 0, st>>>((float4*)links, g, start, seed);
+    else
+        init_kernel<double><<<grid, kBlock, 0, st>>>((double4a*)links, g, start, seed);
+    return 1;
+}
+
+}  // namespace su2

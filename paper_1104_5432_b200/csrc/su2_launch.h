@@ -1,0 +1,41 @@
+// su2_launch.h — host-side launchers shared by the translation units of libsu2hb.so.
+// (Internal to the library; the public boundary is include/su2_heatbath.h.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "su2_device.cuh"
+
+namespace su2 {
+
+// Tile of one CTA of the tiled heat-bath launch, in threads: (hx, y, z, t).
+// Used when every extent is a multiple of the tile (else the linear launch).
+constexpr int kTileLog2[4] = {3, 2, 2, 1};  // 8 x 4 x 4 x 2 = 256 threads, 16 sites along x
+constexpr int kBlock = 256;                 // block size of every other kernel; part of the
+                                            // definition of the fixed-order reductions
+
+struct Scratch {
+    double* partials;   // [device] block partial sums (plaquette | polyakov | correlator)
+    size_t n_partials;  // capacity in doubles
+    double* field;      // [device] l(x) of the Polyakov kernel, V/Nt doubles
+    double* out;        // [device] 2 + kMaxR doubles: plaquette, polyakov, correlator
+    int* err;           // [device] sticky error flags (bit 0: KP trial cap hit)
+};
+constexpr int kMaxR = 128;
+
+bool tiled_ok(const Geom& g);
+size_t partials_needed(const Geom& g);
+
+// each returns the number of kernels it enqueued (0 on launch failure; check cudaGetLastError)
+int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st);
+int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
+                            uint64_t seed, uint32_t sweep, int* err, cudaStream_t st);
+int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
+                     cudaStream_t st);
+int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
+                    cudaStream_t st);
+int launch_polyakov_correlator(const Geom& g, const Scratch& sc, int rmax, double* dev_dst, cudaStream_t st);
+int launch_to_device_layout(const void* canonical, void* links, const Geom& g, int precision, cudaStream_t st);
+int launch_to_canonical(const void* links, void* canonical, const Geom& g, int precision, cudaStream_t st);
+
+}  // namespace su2

@@ -1,0 +1,224 @@
+// su2_measure.cu — mean plaquette (row 7), Polyakov loop (row 8), Polyakov-loop
+// correlator (NEXT-1) and the canonical <-> device layout conversions.
+//
+// Reductions: per-thread fp64 value -> warp shuffle -> fixed-order block tree ->
+// one partial per block -> one final block that sums the partials in a fixed
+// strided order. Block size kBlock is part of the definition, so a given lattice
+// always produces the same bits.
+#include "su2_launch.h"
+
+namespace su2 {
+
+// ------------------------------------------------------------------ plaquette
+// one thread per site; grid.y = parity. [R10]
+//   1/2 Tr[U_mu(x) U_nu(x+mu) U_mu^dag(x+nu) U_nu^dag(x)]
+//     = < U_mu(x) U_nu(x+mu) , U_nu(x) U_mu(x+nu) >   (4-vector dot product)
+template <typename Real>
+__global__ void __launch_bounds__(kBlock)
+    plaquette_kernel(const typename LinkPtr<Real>::type* __restrict__ links, const Geom g,
+                     double* __restrict__ partials)
+{
+    typedef typename LinkPtr<Real>::type L;
+    __shared__ double red[kBlock / 32];
+    const uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
+    const int p = blockIdx.y;
+    double acc = 0.0;
+    if (h < g.vh) {
+        uint32_t q = h / (uint32_t)g.nxh;
+        const int hx = (int)(h - q * (uint32_t)g.nxh);
+        uint32_t q2 = q / (uint32_t)g.n[1];
+        const int y = (int)(q - q2 * (uint32_t)g.n[1]);
+        const int t = (int)(q2 / (uint32_t)g.n[2]);
+        const int z = (int)(q2 - (uint32_t)t * (uint32_t)g.n[2]);
+        const int r = (y + z + t + p) & 1;
+        int up[4];
+        up[0] = r ? ((hx + 1 == g.nxh) ? -(g.nxh - 1) : 1) : 0;
+        up[1] = (y + 1 == g.n[1]) ? -(g.n[1] - 1) * g.sy : g.sy;
+        up[2] = (z + 1 == g.n[2]) ? -(g.n[2] - 1) * g.sz : g.sz;
+        up[3] = (t + 1 == g.n[3]) ? -(g.n[3] - 1) * g.st : g.st;
+        const size_t vh = g.vh;
+        const L* same = links + (size_t)(p * 4) * vh;
+        const L* oppo = links + (size_t)((1 - p) * 4) * vh;
+        Quat<Real> u[4];
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) u[mu] = ldq(same + mu * vh + h);
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu)
+#pragma unroll
+            for (int nu = mu + 1; nu < 4; ++nu) {
+                const Quat<Real> a = qmul<false, false>(u[mu], ldq(oppo + nu * vh + ((int)h + up[mu])));
+                const Quat<Real> b = qmul<false, false>(u[nu], ldq(oppo + mu * vh + ((int)h + up[nu])));
+                acc += (double)qdot(a, b);
+            }
+    }
+    const double tot = block_sum(acc, red);
+    if (threadIdx.x == 0) partials[blockIdx.y * gridDim.x + blockIdx.x] = tot;
+}
+
+// final stage: dst[0] = scale * sum(partials[0..n)), fixed order
+__global__ void __launch_bounds__(1024) final_sum_kernel(const double* __restrict__ partials, size_t n, double scale,
+                                                         double* __restrict__ dst)
+{
+    __shared__ double red[32];
+    double acc = 0.0;
+    for (size_t i = threadIdx.x; i < n; i += 1024) acc += partials[i];
+    const double tot = block_sum(acc, red);
+    if (threadIdx.x == 0) dst[0] = tot * scale;
+}
+
+// ------------------------------------------------------------------ Polyakov loop
+// one thread per spatial site; ordered product of the N_t time links [R11]
+template <typename Real>
+__global__ void __launch_bounds__(kBlock)
+    polyakov_kernel(const typename LinkPtr<Real>::type* __restrict__ links, const Geom g,
+                    double* __restrict__ field, double* __restrict__ partials)
+{
+    typedef typename LinkPtr<Real>::type L;
+    __shared__ double red[kBlock / 32];
+    const uint32_t v3 = (uint32_t)g.n[0] * (uint32_t)g.n[1] * (uint32_t)g.n[2];
+    const uint32_t s3 = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
+    double val = 0.0;
+    if (s3 < v3) {
+        const uint32_t x = s3 % (uint32_t)g.n[0];
+        const uint32_t q = s3 / (uint32_t)g.n[0];
+        const uint32_t y = q % (uint32_t)g.n[1], z = q / (uint32_t)g.n[1];
+        const int p0 = (int)((x + y + z) & 1u);
+        const size_t vh = g.vh;
+        const L* a0 = links + (size_t)(p0 * 4 + 3) * vh + (s3 >> 1);        // even t
+        const L* a1 = links + (size_t)((1 - p0) * 4 + 3) * vh + (s3 >> 1);  // odd t
+        Quat<Real> prod = ldq(a0);
+        for (int t = 1; t < g.n[3]; ++t) {
+            const Quat<Real> u = ldq(((t & 1) ? a1 : a0) + (size_t)t * (size_t)g.st);
+            prod = qmul<false, false>(prod, u);
+        }
+        val = (double)prod.a0;
+        if (field) field[s3] = val;
+    }
+    const double tot = block_sum(val, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+}
+
+// ------------------------------------------------------------------ correlator (NEXT-1)
+// C(r) = 1/(3 V3) sum_x sum_{i=x,y,z} l(x) l(x + r e_i);  grid.y = r-1
+__global__ void __launch_bounds__(kBlock)
+    correlator_kernel(const double* __restrict__ field, const Geom g, double* __restrict__ partials)
+{
+    __shared__ double red[kBlock / 32];
+    const uint32_t v3 = (uint32_t)g.n[0] * (uint32_t)g.n[1] * (uint32_t)g.n[2];
+    const uint32_t s3 = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
+    const int r = blockIdx.y + 1;
+    double val = 0.0;
+    if (s3 < v3) {
+        const int x = (int)(s3 % (uint32_t)g.n[0]);
+        const uint32_t q = s3 / (uint32_t)g.n[0];
+        const int y = (int)(q % (uint32_t)g.n[1]), z = (int)(q / (uint32_t)g.n[1]);
+        const int xs = (x + r) % g.n[0], ys = (y + r) % g.n[1], zs = (z + r) % g.n[2];
+        const double l0 = field[s3];
+        const double lx = field[(uint32_t)xs + (uint32_t)g.n[0] * ((uint32_t)y + (uint32_t)g.n[1] * (uint32_t)z)];
+        const double ly = field[(uint32_t)x + (uint32_t)g.n[0] * ((uint32_t)ys + (uint32_t)g.n[1] * (uint32_t)z)];
+        const double lz = field[(uint32_t)x + (uint32_t)g.n[0] * ((uint32_t)y + (uint32_t)g.n[1] * (uint32_t)zs)];
+        val = l0 * lx + l0 * ly + l0 * lz;
+    }
+    const double tot = block_sum(val, red);
+    if (threadIdx.x == 0) partials[blockIdx.y * gridDim.x + blockIdx.x] = tot;
+}
+__global__ void __launch_bounds__(1024)
+    correlator_final_kernel(const double* __restrict__ partials, size_t n_per_r, double scale, double* __restrict__ dst)
+{
+    __shared__ double red[32];
+    const double* src = partials + (size_t)blockIdx.x * n_per_r;
+    double acc = 0.0;
+    for (size_t i = threadIdx.x; i < n_per_r; i += 1024) acc += src[i];
+    const double tot = block_sum(acc, red);
+    if (threadIdx.x == 0) dst[blockIdx.x] = tot * scale;
+}
+
+// ------------------------------------------------------------------ layout conversion
+// canonical [s][mu] <-> device [p][mu][h]; one thread per (s, mu)
+template <typename Real, bool TO_DEVICE>
+__global__ void __launch_bounds__(kBlock)
+    layout_kernel(typename LinkPtr<Real>::type* __restrict__ canonical, typename LinkPtr<Real>::type* __restrict__ links,
+                  const Geom g)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
+    const uint64_t nlinks = 8ull * g.vh;
+    if (i >= nlinks) return;
+    const uint32_t s = (uint32_t)(i >> 2);
+    const int mu = (int)(i & 3);
+    const uint32_t x = s % (uint32_t)g.n[0];
+    uint32_t q = s / (uint32_t)g.n[0];
+    const uint32_t y = q % (uint32_t)g.n[1];
+    q /= (uint32_t)g.n[1];
+    const uint32_t z = q % (uint32_t)g.n[2], t = q / (uint32_t)g.n[2];
+    const int p = (int)((x + y + z + t) & 1u);
+    typename LinkPtr<Real>::type* dev = links + (size_t)(p * 4 + mu) * g.vh + (s >> 1);
+    if (TO_DEVICE) *dev = canonical[i];
+    else canonical[i] = *dev;
+}
+
+// ------------------------------------------------------------------ launchers
+static inline unsigned blocks_for(uint64_t n) { return (unsigned)((n + kBlock - 1) / kBlock); }
+
+size_t partials_needed(const Geom& g)
+{
+    const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
+    size_t a = 2 * (size_t)blocks_for(g.vh);
+    size_t b = (size_t)kMaxR * blocks_for(v3);
+    return a > b ? a : b;
+}
+
+int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
+                     cudaStream_t st)
+{
+    const dim3 grid(blocks_for(g.vh), 2);
+    if (precision == 32)
+        plaquette_kernel<float><<<grid, kBlock, 0, st>>>((const float4*)links, g, sc.partials);
+    else
+        plaquette_kernel<double><<<grid, kBlock, 0, st>>>((const double4a*)links, g, sc.partials);
+    const double scale = 1.0 / (6.0 * 2.0 * (double)g.vh);
+    final_sum_kernel<<<1, 1024, 0, st>>>(sc.partials, (size_t)grid.x * 2, scale, dev_dst);
+    return 2;
+}
+
+int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
+                    cudaStream_t st)
+{
+    const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
+    const unsigned grid = blocks_for(v3);
+    if (precision == 32)
+        polyakov_kernel<float><<<grid, kBlock, 0, st>>>((const float4*)links, g, sc.field, sc.partials);
+    else
+        polyakov_kernel<double><<<grid, kBlock, 0, st>>>((const double4a*)links, g, sc.field, sc.partials);
+    final_sum_kernel<<<1, 1024, 0, st>>>(sc.partials, grid, 1.0 / (double)v3, dev_dst);
+    return 2;
+}
+
+int launch_polyakov_correlator(const Geom& g, const Scratch& sc, int rmax, double* dev_dst, cudaStream_t st)
+{
+    const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
+    const dim3 grid(blocks_for(v3), (unsigned)rmax);
+    correlator_kernel<<<grid, kBlock, 0, st>>>(sc.field, g, sc.partials);
+    correlator_final_kernel<<<(unsigned)rmax, 1024, 0, st>>>(sc.partials, grid.x, 1.0 / (3.0 * (double)v3), dev_dst);
+    return 2;
+}
+
+int launch_to_device_layout(const void* canonical, void* links, const Geom& g, int precision, cudaStream_t st)
+{
+    const unsigned grid = blocks_for(8ull * g.vh);
+    if (precision == 32)
+        layout_kernel<float, true><<<grid, kBlock, 0, st>>>((float4*)canonical, (float4*)links, g);
+    else
+        layout_kernel<double, true><<<grid, kBlock, 0, st>>>((double4a*)canonical, (double4a*)links, g);
+    return 1;
+}
+int launch_to_canonical(const void* links, void* canonical, const Geom& g, int precision, cudaStream_t st)
+{
+    const unsigned grid = blocks_for(8ull * g.vh);
+    if (precision == 32)
+        layout_kernel<float, false><<<grid, kBlock, 0, st>>>((float4*)canonical, (float4*)links, g);
+    else
+        layout_kernel<double, false><<<grid, kBlock, 0, st>>>((double4a*)canonical, (double4a*)links, g);
+    return 1;
+}
+
+}  // namespace su2

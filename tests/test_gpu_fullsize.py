@@ -1,0 +1,67 @@
+"""Full-size parity (-m gpu) in the launch configuration bench.py times: 32^4 and
+64^4 are too big for a full oracle sweep inside a test, so outputs are sampled and
+recomputed one by one by the oracle from the pre-update configuration, and the
+size-independent properties (unit norm, untouched links, plaquette) are checked."""
+import numpy as np
+import pytest
+
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL = {64: 1e-12, 32: 1e-5}
+FLIP = {64: 1e-11, 32: 1e-5}
+MODE = {64: "f64", 32: "f32"}
+
+
+@pytest.mark.parametrize("dims,prec,start,beta", [
+    ((32, 32, 32, 32), 32, "hot", 6.0),
+    ((32, 32, 32, 32), 64, "hot", 6.0),
+    ((64, 64, 64, 64), 32, "cold", 6.0),
+    ((64, 64, 64, 64), 64, "cold", 6.0),
+    ((48, 48, 48, 6), 64, "hot", 2.5),
+])
+def test_sampled_link_parity_at_bench_sizes(dims, prec, start, beta):
+    import paper_1104_5432_b200 as pkg
+    mode = MODE[prec]
+    seed = 1
+    lat = pkg.Lattice(dims, prec)
+    lat.init(start, seed)
+    lat.sweep(beta, 0)
+    lat.sweep(beta, 1)  # a cold start needs a sweep to become non-trivial
+    before = lat.get_links()
+    V = oracle.volume(dims)
+    rng = np.random.default_rng(5)
+    n_sample = 600
+    s_all = np.arange(V)
+    par_of = lambda s: (s % dims[0] + s // dims[0] % dims[1] + s // (dims[0] * dims[1]) % dims[2]
+                        + s // (dims[0] * dims[1] * dims[2])) % 2
+    # plaquette at full size against the oracle (one pass, fp64 accumulate both sides)
+    P_gpu = lat.mean_plaquette()
+    if V <= 32**4:
+        assert abs(P_gpu - oracle.mean_plaquette(dims, before, mode)) < (1e-12 if prec == 64 else 1e-6)
+    flips = 0
+    for mu, p in ((0, 0), (1, 1), (2, 0), (3, 1)):
+        lat.set_links(before)
+        lat.substep(beta, 2, mu, p)
+        after = lat.get_links()
+        # corners, faces (periodic wrap) and random interior sites of parity p
+        cand = np.concatenate([rng.integers(0, V, size=4 * n_sample), [0, V - 1, dims[0] - 1, V - dims[0]],
+                               np.arange(0, 2 * dims[0]), V - 1 - np.arange(0, 2 * dims[0])])
+        cand = np.unique(cand[par_of(cand) == p])[: n_sample + 2 * dims[0]]
+        for s in cand:
+            u, tr, mg = oracle.heatbath_link(dims, before, beta, seed, 2, int(s), mu, mode)
+            d = np.abs(after[s, mu].astype(np.float64) - u.astype(np.float64)).max()
+            if d > TOL[prec]:
+                assert mg < FLIP[prec], (s, mu, d, mg)
+                flips += 1
+        # properties that hold at any size
+        mask = np.ones((V, 4), bool)
+        mask[par_of(s_all) == p, mu] = False
+        assert (after[mask] == before[mask]).all()
+        upd = after[~mask].astype(np.float64)
+        assert np.abs((upd**2).sum(-1) - 1).max() < (9e-16 if prec == 64 else 2.4e-7)
+        assert np.abs(after[~mask] - before[~mask]).max() > 1e-3
+        del after
+    assert flips <= (0 if prec == 64 else 2)
+    lat.close()

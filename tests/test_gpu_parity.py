@@ -1,0 +1,283 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C-ABI
+binding, against the CPU oracle on the same seeded inputs, element by element.
+
+Tolerances (BASELINE.json north_star): links after one sweep |d| <= 1e-12 (fp64),
+1e-5 (fp32); per-sweep mean plaquette 1e-12 (fp64), 1e-6 (fp32). A link outside
+tolerance is excused only as a rounding-flipped accept decision: the oracle's
+smallest accept margin for that link must be < 1e-11 (fp64) / 1e-5 (fp32), and
+the count of such links must be of the expected order (DESIGN.md §3 [R13])."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1104_5432_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL = {64: 1e-12, 32: 1e-5}
+PTOL = {64: 1e-12, 32: 1e-6}
+FLIP_MARGIN = {64: 1e-11, 32: 1e-5}
+MODE = {64: "f64", 32: "f32"}
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+    assert torch.cuda.is_available(), "-m gpu tests need a CUDA device"
+    import paper_1104_5432_b200 as p
+    p.lib()
+    return p
+
+
+def assert_links_match(gpu, ora, prec, margin=None, max_flips=0, what=""):
+    d = np.abs(gpu.astype(np.float64) - ora.astype(np.float64)).max(-1)
+    bad = d > TOL[prec]
+    nbad = int(bad.sum())
+    if nbad == 0:
+        return 0
+    assert margin is not None, f"{what}: {nbad} links differ, max {d.max():.3e}"
+    assert (margin[bad] < FLIP_MARGIN[prec]).all(), \
+        f"{what}: {nbad} links differ beyond tolerance without a marginal accept decision (max {d.max():.3e})"
+    assert nbad <= max_flips, f"{what}: {nbad} flipped accept decisions, expected <= {max_flips}"
+    return nbad
+
+
+# dims: tiled path (extents multiples of the 16x4x4x2 tile), linear path, ragged, minimal
+SHAPES = [(16, 8, 8, 4), (32, 4, 4, 2), (8, 8, 8, 8), (6, 4, 10, 2), (2, 2, 2, 2), (4, 2, 6, 2)]
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", SHAPES)
+def test_init_matches_oracle(pkg, dims, prec):
+    lat = pkg.Lattice(dims, prec)
+    lat.init("cold", 5)
+    g = lat.get_links()
+    assert (g[..., 0] == 1).all() and (g[..., 1:] == 0).all()
+    assert lat.mean_plaquette() == 1.0 and lat.polyakov_loop() == 1.0
+    lat.init("hot", 5)
+    g = lat.get_links()
+    o = oracle.init(dims, "hot", 5, MODE[prec])
+    # uniforms are bit-identical; only sqrt/sincos rounding differs
+    assert np.abs(g.astype(np.float64) - o.astype(np.float64)).max() < (4e-16 if prec == 64 else 2.4e-7)
+    lat.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_set_get_roundtrip_is_bit_exact(pkg, prec):
+    dims = (6, 4, 10, 2)
+    L = workloads.random_links(dims, 3, np.float64 if prec == 64 else np.float32)
+    lat = pkg.Lattice(dims, prec)
+    lat.set_links(L)
+    assert (lat.get_links() == L).all()
+    lat.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", SHAPES)
+def test_every_substep_matches_oracle_teacher_forced(pkg, dims, prec):
+    mode = MODE[prec]
+    beta, seed, sweep = 2.3, 11, 4
+    L = workloads.random_links(dims, 21, oracle.dtype(mode))
+    lat = pkg.Lattice(dims, prec)
+    lat.set_seed(seed)
+    V = oracle.volume(dims)
+    for mu in range(4):
+        for p in range(2):
+            lat.set_links(L)  # teacher forcing: same input on both sides
+            lat.substep(beta, sweep, mu, p)
+            g = lat.get_links()
+            o = L.copy()
+            mg = np.ones((V, 4))
+            oracle.heatbath_substep(dims, o, beta, seed, sweep, mu, p, mode, margin=mg)
+            assert_links_match(g, o, prec, mg, max_flips=0 if prec == 64 else 1, what=f"mu={mu} p={p}")
+            # only the links of this sub-step changed
+            untouched = np.ones((V, 4), bool)
+            s = np.arange(V)
+            par = (s % dims[0] + s // dims[0] % dims[1] + s // (dims[0] * dims[1]) % dims[2]
+                   + s // (dims[0] * dims[1] * dims[2])) % 2
+            untouched[par == p, mu] = False
+            assert (g[untouched] == L[untouched]).all()
+            L = o  # continue from the oracle's state
+    lat.close()
+
+
+@pytest.mark.parametrize("eps,beta", [(0.05, 6.0), (0.3, 2.3)])
+@pytest.mark.parametrize("prec", [64, 32])
+def test_sweep_on_smooth_lattice_matches_oracle(pkg, prec, eps, beta):
+    """Thermalised-like inputs (large staple norm, alpha ~ 30 at beta = 6)."""
+    dims = (16, 8, 8, 4)
+    mode = MODE[prec]
+    L = workloads.smooth_links(dims, 9, eps, oracle.dtype(mode))
+    lat = pkg.Lattice(dims, prec)
+    lat.set_links(L)
+    lat.set_seed(77)
+    lat.sweep(beta, 3)
+    g = lat.get_links()
+    mg = np.ones((oracle.volume(dims), 4))
+    oracle.heatbath_sweep(dims, L, beta, 77, 3, mode, margin=mg)
+    assert_links_match(g, L, prec, mg, max_flips=0 if prec == 64 else 1)
+    assert abs(lat.mean_plaquette() - oracle.mean_plaquette(dims, L, mode)) < PTOL[prec]
+    lat.close()
+
+
+def test_config1_ten_sweeps_links_and_plaquette(pkg):
+    """BASELINE.json configs[0]: 8^4 fp64, hot start seed 1, beta 2.3, 10 sweeps,
+    plaquette after each; teacher-forced link parity AND free-running plaquette."""
+    w = workloads.C1
+    dims = w.dims
+    L = oracle.init(dims, "hot", w.seed)
+    lat = pkg.Lattice(dims, 64)
+    free = pkg.Lattice(dims, 64)
+    free.init("hot", w.seed)
+    lat.set_seed(w.seed)
+    for i in range(w.sweeps):
+        lat.set_links(L)
+        lat.sweep(w.betas[0], i)
+        free.sweep(w.betas[0], i)
+        oracle.heatbath_sweep(dims, L, w.betas[0], w.seed, i)
+        assert_links_match(lat.get_links(), L, 64, what=f"sweep {i}")
+        P = oracle.mean_plaquette(dims, L)
+        assert abs(lat.mean_plaquette() - P) < 1e-12
+        # in fp64 no accept decision flips (probability ~1e-16 per link), so the
+        # free-running trajectory stays on the oracle's
+        assert abs(free.mean_plaquette() - P) < 1e-12
+        assert abs(free.polyakov_loop() - oracle.polyakov_loop(dims, L)) < 1e-12
+    assert_links_match(free.get_links(), L, 64, what="free-running after 10 sweeps")
+    lat.close()
+    free.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_fp32_and_fp64_ten_sweeps_16c4_teacher_forced(pkg, prec):
+    """configs[1] shape (16^3 x 4), several teacher-forced sweeps with P and L each."""
+    dims = (16, 16, 16, 4)
+    mode = MODE[prec]
+    L = oracle.init(dims, "hot", 100, mode)
+    lat = pkg.Lattice(dims, prec)
+    lat.set_seed(100)
+    V = oracle.volume(dims)
+    flips = 0
+    for i in range(4):
+        lat.set_links(L)
+        lat.sweep(2.4, i)
+        mg = np.ones((V, 4))
+        before = L.copy()
+        oracle.heatbath_sweep(dims, L, 2.4, 100, i, mode, margin=mg)
+        g = lat.get_links()
+        n = assert_links_match(g, L, prec, mg, max_flips=0 if prec == 64 else 40, what=f"sweep {i}")
+        flips += n
+        if n == 0:
+            P, Lp = lat.measure()
+            assert abs(P - oracle.mean_plaquette(dims, L, mode)) < PTOL[prec]
+            assert abs(Lp - oracle.polyakov_loop(dims, L, mode)) < PTOL[prec] * 10
+        del before
+    assert flips <= 40
+    lat.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", SHAPES + [(12, 6, 4, 6)])
+def test_plaquette_and_polyakov_match_oracle(pkg, dims, prec):
+    mode = MODE[prec]
+    L = workloads.random_links(dims, 31, oracle.dtype(mode))
+    lat = pkg.Lattice(dims, prec)
+    lat.set_links(L)
+    tol = 1e-14 if prec == 64 else 2e-7
+    assert abs(lat.mean_plaquette() - oracle.mean_plaquette(dims, L, mode)) < tol
+    assert abs(lat.polyakov_loop() - oracle.polyakov_loop(dims, L, mode)) < tol
+    P, Lp = lat.measure()
+    assert P == lat.mean_plaquette() and Lp == lat.polyakov_loop()  # fixed-order reduction: same bits
+    # smooth lattice: values near 1 test the relative accuracy
+    S = workloads.smooth_links(dims, 32, 0.1, oracle.dtype(mode))
+    lat.set_links(S)
+    assert abs(lat.mean_plaquette() - oracle.mean_plaquette(dims, S, mode)) < tol
+    assert abs(lat.polyakov_loop() - oracle.polyakov_loop(dims, S, mode)) < tol
+    lat.close()
+
+
+def test_gauge_invariance_on_gpu(pkg):
+    dims = (8, 8, 8, 4)
+    L = oracle.init(dims, "hot", 2)
+    G = L.copy()
+    oracle.gauge_transform(dims, G, 5)
+    lat = pkg.Lattice(dims, 64)
+    lat.set_links(L)
+    a = lat.measure()
+    lat.set_links(G)
+    b = lat.measure()
+    assert abs(a[0] - b[0]) < 1e-14 and abs(a[1] - b[1]) < 1e-14
+    lat.close()
+
+
+def test_polyakov_correlator_matches_direct_definition(pkg):
+    dims = (12, 8, 10, 4)
+    L = oracle.init(dims, "hot", 8)
+    for i in range(2):
+        oracle.heatbath_sweep(dims, L, 2.6, 8, i)
+    _, field = oracle.polyakov_loop(dims, L, return_field=True)
+    f = field.reshape(dims[2], dims[1], dims[0])  # [z][y][x]
+    lat = pkg.Lattice(dims, 64)
+    lat.set_links(L)
+    got = lat.polyakov_correlator(4)
+    for r in range(1, 5):
+        want = sum((f * np.roll(f, -r, axis=ax)).mean() for ax in (2, 1, 0)) / 3.0
+        assert abs(got[r - 1] - want) < 1e-14
+    with pytest.raises(pkg.SU2Error):
+        lat.polyakov_correlator(5)  # > min extent / 2
+    lat.close()
+
+
+def test_reproducible_and_sweep_idx_matters(pkg):
+    dims = (16, 8, 8, 4)
+    a = pkg.Lattice(dims, 32)
+    b = pkg.Lattice(dims, 32)
+    for lat in (a, b):
+        lat.init("hot", 9)
+    a.sweep(2.3, 0)
+    b.sweep(2.3, 0)
+    ga, gb = a.get_links(), b.get_links()
+    assert (ga == gb).all()
+    b.init("hot", 9)
+    b.sweep(2.3, 1)
+    assert np.abs(b.get_links() - ga).max() > 0.1
+    a.close()
+    b.close()
+
+
+def test_error_paths_on_gpu(pkg):
+    lat = pkg.Lattice((4, 4, 4, 4), 64)
+    with pytest.raises(pkg.SU2Error) as e:
+        lat.sweep(2.3, 0)  # before init
+    assert e.value.code == pkg.SU2_ESTATE
+    lat.init("cold", 1)
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(pkg.SU2Error) as e:
+            lat.sweep(bad, 0)
+        assert e.value.code == pkg.SU2_EARG
+    with pytest.raises(pkg.SU2Error):
+        lat.substep(2.3, 0, 4, 0)
+    with pytest.raises(AssertionError):
+        pkg.su2_set_links(lat.h, np.zeros((3, 4, 4))[:, ::2])  # non-contiguous rejected by the binding
+    import ctypes as C
+    buf = np.zeros(10)
+    assert pkg.lib().su2_set_links(lat.h, C.c_void_p(buf.ctypes.data), buf.nbytes) == pkg.SU2_EARG
+    lat.sweep(2.3, 0)  # still usable after argument errors
+    assert 0.0 < lat.mean_plaquette() <= 1.0
+    lat.close()
+    # library-owned memory variant
+    h = pkg.su2_lattice_create(4, 4, 4, 4, 32)
+    pkg.su2_init(h, pkg.SU2_START_COLD, 0)
+    assert pkg.su2_mean_plaquette(h) == 1.0
+    pkg.su2_lattice_destroy(h)
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_unit_norm_invariant_after_sweeps(pkg, prec):
+    dims = (16, 8, 8, 8)
+    lat = pkg.Lattice(dims, prec)
+    lat.init("hot", 3)
+    for i in range(5):
+        lat.sweep(6.0, i)
+    g = lat.get_links().astype(np.float64)
+    assert np.abs((g**2).sum(-1) - 1).max() < (9e-16 if prec == 64 else 2.4e-7)
+    lat.close()
