@@ -1,0 +1,366 @@
+#!/usr/bin/env python
+"""bench.py — SU(2) heat-bath throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload C5_64^4|C3_32^4|...] [--precision 32|64] [--headline-only]
+
+A "step" is one pass of the whole hot path over one lattice: one heat-bath sweep
+(8 checkerboard sub-steps), then the mean plaquette and the Polyakov loop of the
+new configuration (the paper's loop: "100 iterations of the heat bath method and
+the calculation of the mean average plaquette at each iteration").
+The random initialisation (row 1) runs once before the warm-up and is reported
+separately as `init_ms`. value = link updates/s = 4V * steps / time.
+
+Headline workload (N=1): BASELINE.json configs[4], 64^4 at beta = 6.0 from a cold
+start in fp32 — the HBM-bound point of the metric ("link updates/s (fp32/fp64) at
+32^4 and 64^4; % of HBM roofline"); the other three points of the metric (64^4
+fp64, 32^4 fp32/fp64) are timed the same way and reported under "workloads".
+The path does not shard (north_star: no multi-GPU path): with --gpus N every rank
+runs an independent replica (different seed), no collective on the data path.
+
+--impl reference times the CPU oracle as it stands on the host cores.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "su2_heatbath_link_updates_per_s"
+UNIT = "link updates/s"
+BYTES_PER_UPDATE = {32: 128, 64: 256}  # 8 quaternions per link update
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            with open(path) as f:
+                return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def mark(self):
+        return time.time()
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self, t0, t1):
+        sm, smax, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for t, line in self.rows:
+            if t < t0 or t > t1 + 0.15:
+                continue
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0]))
+                smax = max(smax, float(f[1]))
+                for n, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": smax, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# ------------------------------------------------------------------------------- ours
+def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, dist=None):
+    """Device-resident timing of `steps` steps. Returns a dict of measurements."""
+    lat = pkg.Lattice(w.dims, prec)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    obs = torch.zeros(2 * (steps + warmup), dtype=torch.float64, device=lat.device)
+
+    e0, e1 = ev(), ev()
+    torch.cuda.synchronize()
+    e0.record()
+    lat.init(w.start, seed)
+    e1.record()
+    torch.cuda.synchronize()
+    init_ms = e0.elapsed_time(e1)
+
+    def step(i):
+        lat.sweep(beta, i)
+        lat.measure_async(obs, i)
+
+    for i in range(warmup):
+        step(i)
+    lat.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    n0 = lat.launch_count
+    sweep_ev = [(ev(), ev()) for _ in range(steps)]
+    t_wall0 = sampler.mark() if sampler else 0.0
+    start, stop = ev(), ev()
+    start.record()
+    for k in range(steps):
+        i = warmup + k
+        sweep_ev[k][0].record()
+        lat.sweep(beta, i)
+        sweep_ev[k][1].record()
+        lat.measure_async(obs, i)
+    stop.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t_wall1 = sampler.mark() if sampler else 0.0
+    lat.synchronize()  # surfaces device-side error flags
+    launches = lat.launch_count - n0
+    ms = start.elapsed_time(stop)
+    sweep_ms = float(np.mean([a.elapsed_time(b) for a, b in sweep_ev]))
+    o = obs.cpu().numpy().reshape(-1, 2)
+    res = {
+        "ms_total": ms, "ms_per_step": ms / steps, "sweep_ms": sweep_ms, "init_ms": init_ms,
+        "launches": int(launches), "plaquette_last": float(o[warmup + steps - 1, 0]),
+        "polyakov_last": float(o[warmup + steps - 1, 1]), "t_wall": (t_wall0, t_wall1),
+        "links": w.links,
+    }
+    lat.close()
+    del lat, obs
+    torch.cuda.empty_cache()
+    return res
+
+
+def time_e2e(pkg, torch, w, prec, beta, steps, warmup, seed):
+    """Same step through the C-ABI with HOST buffers: every step copies the input
+    configuration host->device (su2_set_links, pinned), runs sweep + plaquette +
+    Polyakov, and reads the new configuration and the observables back
+    (su2_get_links + su2_measure)."""
+    lat = pkg.Lattice(w.dims, prec)
+    nbytes = pkg.su2_lattice_bytes(*w.dims, prec)
+    dt = np.float32 if prec == 32 else np.float64
+    pinned = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    host = pinned.numpy().view(dt).reshape(w.volume, 4, 4)
+    lat.init(w.start, seed)
+    lat.get_links(host)
+    t = []
+    for k in range(warmup + steps):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        lat.set_links(host)
+        lat.sweep(beta, k)
+        P, L = lat.measure()
+        lat.get_links(host)
+        torch.cuda.synchronize()
+        t.append(time.perf_counter() - t0)
+    lat.close()
+    sec = float(np.mean(t[warmup:]))
+    return {"value": w.links / sec, "unit": UNIT, "h2d_bytes_per_step": int(nbytes),
+            "d2h_bytes_per_step": int(nbytes + 16), "ms_per_step": sec * 1e3, "steps": steps,
+            "what": "su2_set_links(pinned host) + su2_heatbath_sweep + su2_measure + su2_get_links(pinned host)"}
+
+
+# ------------------------------------------------------------------------------- oracle
+def oracle_sample(w, prec, beta, seed, n_substeps=2):
+    """The oracle as it stands on one host core: the first `n_substeps` sub-steps
+    (mu=0; parity 0,1) of sweep 0 on the workload's own lattice."""
+    import oracle
+    mode = "f32" if prec == 32 else "f64"
+    links = oracle.init(w.dims, w.start, seed, mode)
+    t0 = time.perf_counter()
+    done = 0
+    for j in range(n_substeps):
+        oracle.heatbath_substep(w.dims, links, beta, seed, 0, j // 2, j % 2, mode)
+        done += w.volume // 2
+    sec = time.perf_counter() - t0
+    return done / sec, sec, done
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    from paper_1104_5432_b200 import workloads
+    w = workloads.BY_NAME[args.workload]
+    prec = args.precision
+    # bounded sample per step: one sub-step pair on 32^4-sized work (the 64^4 lattice itself for C5)
+    vals, secs, n = [], [], 0
+    for k in range(args.warmup + args.steps):
+        v, s, n = oracle_sample(w, prec, args.beta, args.seed, n_substeps=args.ref_substeps)
+        if k >= args.warmup:
+            vals.append(v)
+            secs.append(s)
+    value = float(np.mean(vals))
+    sample = (f"{args.ref_substeps} heat-bath sub-step(s) (mu=0) of sweep 0 on the {w.name} lattice "
+              f"({n} link updates per step), fp{prec} oracle mode, gcc -O2, serial")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(secs)) * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
+        "config": {"workload": f"{w.name} beta={args.beta} start={w.start} (bounded sample)", "precision": prec},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------- main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C5_64^4")
+    ap.add_argument("--precision", type=int, default=32, choices=[32, 64])
+    ap.add_argument("--beta", type=float, default=6.0)
+    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--headline-only", action="store_true", help="skip the other metric points, e2e and cpu_baseline")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--ref-substeps", type=int, default=2)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.warmup < 3:
+        args.warmup = 3  # timing rule: W >= 3
+
+    import torch
+    from paper_1104_5432_b200 import workloads
+    import paper_1104_5432_b200 as pkg
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    pkg.lib()
+    peak, peak_src = measured_peaks()
+    w = workloads.BY_NAME[args.workload]
+    prec = args.precision
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    r = time_workload(pkg, torch, w, prec, args.beta, args.steps, args.warmup, args.seed + rank, sampler, dist)
+    clocks = sampler.summary(*r["t_wall"])
+
+    ms = r["ms_total"]
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * w.links * args.steps / (ms * 1e-3)
+
+    # roofline of the dominant kernel (heat-bath sub-step): algorithmic bytes per launch =
+    # (V/2 updates) * 8 quaternions; duration = sweep time / 8 launches, CUDA events on the
+    # launching stream inside the timed region.
+    sub_s = r["sweep_ms"] * 1e-3 / 8.0
+    alg_bytes = (w.volume // 2) * BYTES_PER_UPDATE[prec]
+    achieved = alg_bytes / sub_s / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "kernel": "heatbath sub-step (one per (mu,parity))",
+                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_us": sub_s * 1e6}
+    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(prof):
+        try:
+            with open(prof) as f:
+                roofline["traffic"] = json.load(f).get(f"{w.name}_fp{prec}")
+        except Exception:
+            pass
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
+        "config": {"workload": f"{w.name} beta={args.beta} start={w.start} seed={args.seed}",
+                   "precision": prec, "step": "1 heat-bath sweep (8 sub-steps) + mean plaquette + Polyakov loop",
+                   "l2": ("inputs larger than L2 (%d MiB lattice)" % (w.links * 4 * prec // 8 >> 20)),
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "clocks": clocks, "gpu_launches": r["launches"], "roofline": roofline,
+        "sweep_only": {"value": world * w.links / (r["sweep_ms"] * 1e-3), "unit": UNIT, "ms_per_sweep": r["sweep_ms"]},
+        "init_ms": r["init_ms"], "plaquette_last": r["plaquette_last"], "polyakov_last": r["polyakov_last"],
+    }
+
+    if not args.headline_only and rank == 0:
+        # the other points of the metric, device-resident, same step
+        others = {}
+        for name, p in (("C5_64^4", 64), ("C3_32^4", 32), ("C3_32^4", 64)):
+            if name == w.name and p == prec:
+                continue
+            ww = workloads.BY_NAME[name]
+            rr = time_workload(pkg, torch, ww, p, args.beta, args.steps, args.warmup, args.seed)
+            ss = rr["sweep_ms"] * 1e-3 / 8.0
+            ach = (ww.volume // 2) * BYTES_PER_UPDATE[p] / ss / 1e9
+            lattice_mib = ww.links * 4 * p // 8 >> 20
+            others[f"{name}_fp{p}"] = {
+                "value": ww.links * args.steps / (rr["ms_total"] * 1e-3), "unit": UNIT,
+                "ms_per_step": rr["ms_per_step"], "ms_per_sweep": rr["sweep_ms"],
+                "roofline_frac_hbm": ach / peak, "achieved_gbs": ach,
+                "note": ("lattice %d MiB: L2-resident, HBM peak is not its bound" % lattice_mib) if lattice_mib <= 126
+                else ("lattice %d MiB > L2" % lattice_mib),
+                "plaquette_last": rr["plaquette_last"],
+            }
+        line["workloads"] = others
+        line["e2e"] = time_e2e(pkg, torch, w, prec, args.beta, args.e2e_steps, 1, args.seed)
+        v, sec, n = oracle_sample(w, prec, args.beta, args.seed, n_substeps=args.ref_substeps)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"{args.ref_substeps} heat-bath sub-steps (mu=0, both parities) of sweep 0 on "
+                                          f"the {w.name} lattice = {n} link updates in {sec:.1f} s, fp{prec} oracle "
+                                          f"mode, gcc -O2, serial"}
+    sampler.stop()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

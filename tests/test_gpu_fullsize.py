@@ -60,7 +60,7 @@ def test_sampled_link_parity_at_bench_sizes(dims, prec, start, beta):
         mask[par_of(s_all) == p, mu] = False
         assert (after[mask] == before[mask]).all()
         upd = after[~mask].astype(np.float64)
-        assert np.abs((upd**2).sum(-1) - 1).max() < (9e-16 if prec == 64 else 2.4e-7)
+        assert np.abs((upd**2).sum(-1) - 1).max() < (9e-16 if prec == 64 else 5e-7)  # 4 ulp on |a|^2
         assert np.abs(after[~mask] - before[~mask]).max() > 1e-3
         del after
     assert flips <= (0 if prec == 64 else 2)
