@@ -286,7 +286,9 @@ def main():
 
     sampler = ClockSampler(local)
     sampler.start()
-    time.sleep(0.3)
+    t_wait = time.time()
+    while not sampler.rows and time.time() - t_wait < 5.0:  # nvidia-smi takes ~1 s to emit its first line
+        time.sleep(0.05)
     r = time_workload(pkg, torch, w, prec, args.beta, args.steps, args.warmup, args.seed + rank, sampler, dist)
     clocks = sampler.summary(*r["t_wall"])
 
@@ -320,7 +322,10 @@ def main():
         "vs_baseline": None, "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
         "config": {"workload": f"{w.name} beta={args.beta} start={w.start} seed={args.seed}",
                    "precision": prec, "step": "1 heat-bath sweep (8 sub-steps) + mean plaquette + Polyakov loop",
-                   "l2": ("inputs larger than L2 (%d MiB lattice)" % (w.links * 4 * prec // 8 >> 20)),
+                   "l2": (("inputs larger than L2 (%d MiB lattice vs 126 MiB L2), no flush needed"
+                           if (w.links * 4 * prec // 8 >> 20) > 126 else
+                           "lattice %d MiB is L2-resident by nature of the workload; no flush between steps")
+                          % (w.links * 4 * prec // 8 >> 20)),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks, "gpu_launches": r["launches"], "roofline": roofline,
         "sweep_only": {"value": world * w.links / (r["sweep_ms"] * 1e-3), "unit": UNIT, "ms_per_sweep": r["sweep_ms"]},

@@ -85,11 +85,17 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
     g.st = g.nxh * Ny * Nz;
     g.vh = (uint32_t)((uint64_t)Nx * Ny * Nz * Nt / 2);
     g.nb[0] = g.nb[1] = g.nb[2] = g.nb[3] = 0;
+    g.wup[0] = -(g.nxh - 1);
+    g.wup[1] = -(Ny - 1) * g.sy;
+    g.wup[2] = -(Nz - 1) * g.sz;
+    g.wup[3] = -(Nt - 1) * g.st;
+    g.zmagic = 0;
     if (tiled_ok(g)) {
         g.nb[0] = g.nxh >> kTileLog2[0];
         g.nb[1] = Ny >> kTileLog2[1];
         g.nb[2] = Nz >> kTileLog2[2];
         g.nb[3] = Nt >> kTileLog2[3];
+        g.zmagic = (uint32_t)(((1ull << 32) + (uint64_t)g.nb[2] - 1) / (uint64_t)g.nb[2]);  // unused if nb2 == 1
     }
     lat->precision = precision;
     lat->stream = (cudaStream_t)stream;

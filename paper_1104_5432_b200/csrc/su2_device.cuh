@@ -19,6 +19,8 @@ struct Geom {
     int sy, sz, st;  // strides of y, z, t in half-index units: nxh, nxh*Ny, nxh*Ny*Nz
     uint32_t vh;     // V/2
     int nb[4];       // tiled launch: number of tiles along hx, y, z, t
+    int wup[4];      // half-index delta of +mu at the upper boundary: -(N-1)*stride  (x: -(nxh-1))
+    uint32_t zmagic; // ceil(2^32 / nb[2]): blockIdx.z -> (bz, bt) without a division
 };
 
 // ---------------------------------------------------------------- quaternions
@@ -69,17 +71,32 @@ __device__ __forceinline__ void stq(double4a* p, const Quat<double>& q)
 
 // [R1] c = op(a) * op(b), op = dagger when DA / DB:
 //   c0 = a0 b0 - a.b ; cvec = a0 b + b0 a - a x b ; dagger flips the vector part.
+// Written as FMA chains (4 mul + 12 fma, sign flips ride on the FMA operands).
+__device__ __forceinline__ float fmad(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fmad(double a, double b, double c) { return fma(a, b, c); }
+
 template <bool DA, bool DB, typename Real>
 __device__ __forceinline__ Quat<Real> qmul(const Quat<Real>& a, const Quat<Real>& b)
 {
     const Real a1 = DA ? -a.a1 : a.a1, a2 = DA ? -a.a2 : a.a2, a3 = DA ? -a.a3 : a.a3;
     const Real b1 = DB ? -b.a1 : b.a1, b2 = DB ? -b.a2 : b.a2, b3 = DB ? -b.a3 : b.a3;
     Quat<Real> c;
-    c.a0 = a.a0 * b.a0 - a1 * b1 - a2 * b2 - a3 * b3;
-    c.a1 = a.a0 * b1 + b.a0 * a1 - (a2 * b3 - a3 * b2);
-    c.a2 = a.a0 * b2 + b.a0 * a2 - (a3 * b1 - a1 * b3);
-    c.a3 = a.a0 * b3 + b.a0 * a3 - (a1 * b2 - a2 * b1);
+    c.a0 = fmad(-a3, b3, fmad(-a2, b2, fmad(-a1, b1, a.a0 * b.a0)));
+    c.a1 = fmad(a3, b2, fmad(-a2, b3, fmad(b.a0, a1, a.a0 * b1)));
+    c.a2 = fmad(a1, b3, fmad(-a3, b1, fmad(b.a0, a2, a.a0 * b2)));
+    c.a3 = fmad(a2, b1, fmad(-a1, b2, fmad(b.a0, a3, a.a0 * b3)));
     return c;
+}
+// acc += op(a) * op(b)   (16 fma)
+template <bool DA, bool DB, typename Real>
+__device__ __forceinline__ void qmac(Quat<Real>& acc, const Quat<Real>& a, const Quat<Real>& b)
+{
+    const Real a1 = DA ? -a.a1 : a.a1, a2 = DA ? -a.a2 : a.a2, a3 = DA ? -a.a3 : a.a3;
+    const Real b1 = DB ? -b.a1 : b.a1, b2 = DB ? -b.a2 : b.a2, b3 = DB ? -b.a3 : b.a3;
+    acc.a0 = fmad(-a3, b3, fmad(-a2, b2, fmad(-a1, b1, fmad(a.a0, b.a0, acc.a0))));
+    acc.a1 = fmad(a3, b2, fmad(-a2, b3, fmad(b.a0, a1, fmad(a.a0, b1, acc.a1))));
+    acc.a2 = fmad(a1, b3, fmad(-a3, b1, fmad(b.a0, a2, fmad(a.a0, b2, acc.a2))));
+    acc.a3 = fmad(a2, b1, fmad(-a1, b2, fmad(b.a0, a3, fmad(a.a0, b3, acc.a3))));
 }
 // scalar part only of a * b^dagger  ( = 4-vector dot product )
 template <typename Real>
@@ -128,6 +145,19 @@ struct M<float> {
     static __device__ __forceinline__ float log(float x) { return logf(x); }
     static __device__ __forceinline__ float sqrt(float x) { return sqrtf(x); }
     static __device__ __forceinline__ float rcp(float x) { return 1.0f / x; }
+    // MUFU approximations (<= 2 ulp): the fp32 link tolerance is 1e-5
+    static __device__ __forceinline__ float rsqrt(float x)
+    {
+        float r;
+        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return r;
+    }
+    static __device__ __forceinline__ float sqrt0(float x)  // x >= 0
+    {
+        float r;
+        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return r;
+    }
     static __device__ __forceinline__ float cos2pi(float x) { return cospif(2.0f * x); }
     static __device__ __forceinline__ void sincos2pi(float x, float* s, float* c) { sincospif(2.0f * x, s, c); }
     static __device__ __forceinline__ float tiny() { return 1e-20f; }
@@ -142,6 +172,8 @@ struct M<double> {
     static __device__ __forceinline__ double log(double x) { return ::log(x); }
     static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
     static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
+    static __device__ __forceinline__ double rsqrt(double x) { return ::rsqrt(x); }
+    static __device__ __forceinline__ double sqrt0(double x) { return x * ::rsqrt(fmax(x, 1e-300)); }  // x >= 0
     static __device__ __forceinline__ double cos2pi(double x) { return cospi(2.0 * x); }
     static __device__ __forceinline__ void sincos2pi(double x, double* s, double* c) { sincospi(2.0 * x, s, c); }
     static __device__ __forceinline__ double tiny() { return 1e-30; }

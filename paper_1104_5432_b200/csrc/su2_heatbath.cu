@@ -22,21 +22,21 @@ struct Nbr {
 __device__ __forceinline__ Nbr neighbours(const Geom& g, const Site& c, int r)
 {
     Nbr d;
-    d.up[0] = r ? ((c.hx + 1 == g.nxh) ? -(g.nxh - 1) : 1) : 0;
-    d.dn[0] = r ? 0 : ((c.hx == 0) ? (g.nxh - 1) : -1);
-    d.up[1] = (c.y + 1 == g.n[1]) ? -(g.n[1] - 1) * g.sy : g.sy;
-    d.dn[1] = (c.y == 0) ? (g.n[1] - 1) * g.sy : -g.sy;
-    d.up[2] = (c.z + 1 == g.n[2]) ? -(g.n[2] - 1) * g.sz : g.sz;
-    d.dn[2] = (c.z == 0) ? (g.n[2] - 1) * g.sz : -g.sz;
-    d.up[3] = (c.t + 1 == g.n[3]) ? -(g.n[3] - 1) * g.st : g.st;
-    d.dn[3] = (c.t == 0) ? (g.n[3] - 1) * g.st : -g.st;
+    d.up[0] = r ? ((c.hx + 1 == g.nxh) ? g.wup[0] : 1) : 0;
+    d.dn[0] = r ? 0 : ((c.hx == 0) ? -g.wup[0] : -1);
+    d.up[1] = (c.y + 1 == g.n[1]) ? g.wup[1] : g.sy;
+    d.dn[1] = (c.y == 0) ? -g.wup[1] : -g.sy;
+    d.up[2] = (c.z + 1 == g.n[2]) ? g.wup[2] : g.sz;
+    d.dn[2] = (c.z == 0) ? -g.wup[2] : -g.sz;
+    d.up[3] = (c.t + 1 == g.n[3]) ? g.wup[3] : g.st;
+    d.dn[3] = (c.t == 0) ? -g.wup[3] : -g.st;
     return d;
 }
 
 template <typename Real, int MU>
 __device__ __forceinline__ void heatbath_site(typename LinkPtr<Real>::type* __restrict__ links, const Geom& g,
-                                              int p, const Site& c, Real beta, uint64_t seed, uint32_t sweep,
-                                              int* __restrict__ err)
+                                              int p, const Site& c, Real beta, Real inv_beta, uint64_t seed,
+                                              uint32_t sweep, int* __restrict__ err)
 {
     typedef typename LinkPtr<Real>::type L;
     const int r = (c.y + c.z + c.t + p) & 1;
@@ -45,22 +45,26 @@ __device__ __forceinline__ void heatbath_site(typename LinkPtr<Real>::type* __re
     const size_t vh = g.vh;
     const L* same = links + (size_t)(p * 4) * vh;        // arrays of parity p
     const L* oppo = links + (size_t)((1 - p) * 4) * vh;  // arrays of parity 1-p
+    const L* o_mu = oppo + MU * vh;                      // U_mu on the other parity
 
-    // [R3] staple sum, nu ascending, forward then backward, products left to right
+    // [R3] staple sum, nu ascending, forward then backward, products left to right;
+    // the second product of every term accumulates straight into v (FMA chains).
     Quat<Real> v = {0, 0, 0, 0};
+    const int h_up = h + d.up[MU];
 #pragma unroll
     for (int nu = 0; nu < 4; ++nu) {
         if (nu == MU) continue;
-        const Quat<Real> a = ldq(oppo + nu * vh + (h + d.up[MU]));             // U_nu(x+mu)
-        const Quat<Real> b = ldq(oppo + MU * vh + (h + d.up[nu]));             // U_mu(x+nu)
-        const Quat<Real> cc = ldq(same + nu * vh + h);                         // U_nu(x)
-        const Quat<Real> a2 = ldq(same + nu * vh + (h + d.up[MU] + d.dn[nu]));  // U_nu(x+mu-nu)
-        const Quat<Real> b2 = ldq(oppo + MU * vh + (h + d.dn[nu]));            // U_mu(x-nu)
-        const Quat<Real> c2 = ldq(oppo + nu * vh + (h + d.dn[nu]));            // U_nu(x-nu)
-        const Quat<Real> f = qmul<false, true>(qmul<false, true>(a, b), cc);
-        const Quat<Real> w = qmul<false, false>(qmul<true, true>(a2, b2), c2);
-        v.a0 += f.a0; v.a1 += f.a1; v.a2 += f.a2; v.a3 += f.a3;
-        v.a0 += w.a0; v.a1 += w.a1; v.a2 += w.a2; v.a3 += w.a3;
+        const L* s_nu = same + nu * vh;
+        const L* o_nu = oppo + nu * vh;
+        const int h_dn = h + d.dn[nu];
+        const Quat<Real> a = ldq(o_nu + h_up);                // U_nu(x+mu)
+        const Quat<Real> b = ldq(o_mu + (h + d.up[nu]));      // U_mu(x+nu)
+        const Quat<Real> cc = ldq(s_nu + h);                  // U_nu(x)
+        const Quat<Real> a2 = ldq(s_nu + (h_up + d.dn[nu]));  // U_nu(x+mu-nu)
+        const Quat<Real> b2 = ldq(o_mu + h_dn);               // U_mu(x-nu)
+        const Quat<Real> c2 = ldq(o_nu + h_dn);               // U_nu(x-nu)
+        qmac<false, true>(v, qmul<false, true>(a, b), cc);    // (a b^+) c^+
+        qmac<false, false>(v, qmul<true, true>(a2, b2), c2);  // (a2^+ b2^+) c2
     }
 
     // [R5] counter = (s, sweep, (p<<2)|mu, n)
@@ -73,8 +77,8 @@ __device__ __forceinline__ void heatbath_site(typename LinkPtr<Real>::type* __re
     if (k2 < M<Real>::tiny()) {  // [R8]
         u = haar_from_words<Real>(wd);
     } else {
-        const Real alpha = beta * M<Real>::sqrt(k2);
-        const Real inv_alpha = M<Real>::rcp(alpha);
+        const Real rk = M<Real>::rsqrt(k2);      // 1/k
+        const Real inv_alpha = rk * inv_beta;    // 1/(beta k)
         // [R6] Kennedy-Pendleton
         Real delta = 0;
         uint32_t n = 1;
@@ -93,44 +97,44 @@ __device__ __forceinline__ void heatbath_site(typename LinkPtr<Real>::type* __re
         }
         // [R7] direction on the sphere of radius sqrt(delta(2-delta)), compose with Vbar^dagger
         const Real x0 = (Real)1 - delta;
-        const Real rad = M<Real>::sqrt(fmax(delta * ((Real)2 - delta), (Real)0));
+        const Real rad = M<Real>::sqrt0(fmax(delta * ((Real)2 - delta), (Real)0));
         const Real cth = (Real)1 - (Real)2 * M<Real>::uniform(wd.w0);
-        const Real sth = M<Real>::sqrt(fmax((Real)1 - cth * cth, (Real)0));
+        const Real sth = M<Real>::sqrt0(fmax((Real)1 - cth * cth, (Real)0));
         Real sphi, cphi;
         M<Real>::sincos2pi(M<Real>::uniform(wd.w1), &sphi, &cphi);
-        const Quat<Real> X = {x0, rad * sth * cphi, rad * sth * sphi, rad * cth};
+        const Real rs = rad * sth;
+        const Quat<Real> X = {x0, rs * cphi, rs * sphi, rad * cth};
         u = qmul<false, true>(X, v);  // X * v^dagger = k * (X * Vbar^dagger); k drops out below
     }
-    const Real inv = M<Real>::rcp(M<Real>::sqrt(u.a0 * u.a0 + u.a1 * u.a1 + u.a2 * u.a2 + u.a3 * u.a3));
+    const Real inv = M<Real>::rsqrt(u.a0 * u.a0 + u.a1 * u.a1 + u.a2 * u.a2 + u.a3 * u.a3);
     u.a0 *= inv; u.a1 *= inv; u.a2 *= inv; u.a3 *= inv;
     stq(links + (size_t)(p * 4 + MU) * vh + h, u);
 }
 
-// tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile
+// tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile;
+// grid = (nb0, nb1, nb2*nb3): x fastest, so CTAs are scheduled roughly in memory order.
 template <typename Real, int MU, int LHX, int LY, int LZ, int LT>
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT))
     heatbath_tiled_kernel(typename LinkPtr<Real>::type* __restrict__ links, const Geom g, int p, Real beta,
-                          uint64_t seed, uint32_t sweep, int* __restrict__ err)
+                          Real inv_beta, uint64_t seed, uint32_t sweep, int* __restrict__ err)
 {
-    int b = blockIdx.x;
-    const int bx = b % g.nb[0]; b /= g.nb[0];
-    const int by = b % g.nb[1]; b /= g.nb[1];
-    const int bz = b % g.nb[2];
-    const int bt = b / g.nb[2];
+    const uint32_t bzt = blockIdx.z;
+    const uint32_t bt = (g.nb[2] == 1) ? bzt : __umulhi(bzt, g.zmagic);
+    const uint32_t bz = bzt - bt * (uint32_t)g.nb[2];
     const int tid = threadIdx.x;
     Site c;
-    c.hx = (bx << LHX) + (tid & ((1 << LHX) - 1));
-    c.y = (by << LY) + ((tid >> LHX) & ((1 << LY) - 1));
-    c.z = (bz << LZ) + ((tid >> (LHX + LY)) & ((1 << LZ) - 1));
-    c.t = (bt << LT) + (tid >> (LHX + LY + LZ));
-    heatbath_site<Real, MU>(links, g, p, c, beta, seed, sweep, err);
+    c.hx = (int)(blockIdx.x << LHX) + (tid & ((1 << LHX) - 1));
+    c.y = (int)(blockIdx.y << LY) + ((tid >> LHX) & ((1 << LY) - 1));
+    c.z = (int)(bz << LZ) + ((tid >> (LHX + LY)) & ((1 << LZ) - 1));
+    c.t = (int)(bt << LT) + (tid >> (LHX + LY + LZ));
+    heatbath_site<Real, MU>(links, g, p, c, beta, inv_beta, seed, sweep, err);
 }
 
 // linear launch: thread i <-> half-index h = i; any even extents
 template <typename Real, int MU>
 __global__ void __launch_bounds__(kBlock)
     heatbath_linear_kernel(typename LinkPtr<Real>::type* __restrict__ links, const Geom g, int p, Real beta,
-                           uint64_t seed, uint32_t sweep, int* __restrict__ err)
+                           Real inv_beta, uint64_t seed, uint32_t sweep, int* __restrict__ err)
 {
     const uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
     if (h >= g.vh) return;
@@ -141,7 +145,7 @@ __global__ void __launch_bounds__(kBlock)
     c.y = (int)(q - q2 * (uint32_t)g.n[1]);
     c.t = (int)(q2 / (uint32_t)g.n[2]);
     c.z = (int)(q2 - (uint32_t)c.t * (uint32_t)g.n[2]);
-    heatbath_site<Real, MU>(links, g, p, c, beta, seed, sweep, err);
+    heatbath_site<Real, MU>(links, g, p, c, beta, inv_beta, seed, sweep, err);
 }
 
 // [R9] init: one thread per link of the device layout
@@ -170,6 +174,10 @@ __global__ void __launch_bounds__(kBlock)
 
 bool tiled_ok(const Geom& g)
 {
+    // grid limits (y, z <= 65535) and exactness of the zmagic split: nb2^2 * nb3 < 2^32
+    const uint64_t t0 = g.nxh >> kTileLog2[0], t1 = g.n[1] >> kTileLog2[1], t2 = g.n[2] >> kTileLog2[2],
+                   t3 = g.n[3] >> kTileLog2[3];
+    if (t1 > 65535 || t2 * t3 > 65535 || t0 == 0) return false;
     return g.nxh % (1 << kTileLog2[0]) == 0 && g.n[1] % (1 << kTileLog2[1]) == 0 &&
            g.n[2] % (1 << kTileLog2[2]) == 0 && g.n[3] % (1 << kTileLog2[3]) == 0;
 }
@@ -181,12 +189,13 @@ static int launch_substep_t(void* links, const Geom& g, int parity, double beta,
     typedef typename LinkPtr<Real>::type L;
     if (tiled_ok(g)) {
         constexpr int T = 1 << (kTileLog2[0] + kTileLog2[1] + kTileLog2[2] + kTileLog2[3]);
-        const unsigned grid = (unsigned)(g.nb[0] * g.nb[1] * g.nb[2] * g.nb[3]);
+        const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
         heatbath_tiled_kernel<Real, MU, kTileLog2[0], kTileLog2[1], kTileLog2[2], kTileLog2[3]>
-            <<<grid, T, 0, st>>>((L*)links, g, parity, (Real)beta, seed, sweep, err);
+            <<<grid, T, 0, st>>>((L*)links, g, parity, (Real)beta, (Real)(1.0 / beta), seed, sweep, err);
     } else {
         const unsigned grid = (g.vh + kBlock - 1) / kBlock;
-        heatbath_linear_kernel<Real, MU><<<grid, kBlock, 0, st>>>((L*)links, g, parity, (Real)beta, seed, sweep, err);
+        heatbath_linear_kernel<Real, MU><<<grid, kBlock, 0, st>>>((L*)links, g, parity, (Real)beta, (Real)(1.0 / beta), seed,
+                                                                  sweep, err);
     }
     return 1;
 }
