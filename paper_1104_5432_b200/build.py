@@ -34,6 +34,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = _nvcc()
     extra = ["-Xptxas", "-v"] if verbose else []
+    extra += os.environ.get("SU2HB_NVCC_EXTRA", "").split()  # tuning sweeps only (e.g. -DHB_MINB_F32=3)
 
     def compile_one(src):
         obj = os.path.join(CSRC, src.replace(".cu", ".o"))

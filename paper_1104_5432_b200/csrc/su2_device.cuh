@@ -47,8 +47,12 @@ struct LinkPtr<double> {
 // read is written, and L1 is invalidated at every launch.
 __device__ __forceinline__ Quat<float> ldq(const float4* p)
 {
-    float4 v = __ldg(p);
-    return {v.x, v.y, v.z, v.w};
+    Quat<float> q;
+    // volatile: keeps the 18 staple loads of a thread in program order, ahead of the arithmetic
+    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(q.a0), "=f"(q.a1), "=f"(q.a2), "=f"(q.a3)
+                 : "l"(p));
+    return q;
 }
 __device__ __forceinline__ Quat<double> ldq(const double4a* p)
 {
@@ -59,13 +63,18 @@ __device__ __forceinline__ Quat<double> ldq(const double4a* p)
                  : "l"(p));
     return q;
 }
+// The updated link is not read again in its own sub-step: streaming store (evict-first in L2).
+#ifndef HB_ST
+#define HB_ST ".cs"
+#endif
 __device__ __forceinline__ void stq(float4* p, const Quat<float>& q)
 {
-    *p = make_float4(q.a0, q.a1, q.a2, q.a3);
+    asm volatile("st.global" HB_ST ".v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(q.a0), "f"(q.a1), "f"(q.a2), "f"(q.a3)
+                 : "memory");
 }
 __device__ __forceinline__ void stq(double4a* p, const Quat<double>& q)
 {
-    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(q.a0), "d"(q.a1), "d"(q.a2), "d"(q.a3)
+    asm volatile("st.global" HB_ST ".v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(q.a0), "d"(q.a1), "d"(q.a2), "d"(q.a3)
                  : "memory");
 }
 
@@ -131,17 +140,47 @@ __device__ __forceinline__ Words draw(uint64_t seed, uint32_t s, uint32_t sweep,
 {
     return philox4x32_10(s, sweep, tag, n, (uint32_t)seed, (uint32_t)(seed >> 32));
 }
+// The 10 round keys depend on the seed only: the launcher expands them once on the
+// host (same Weyl sequence as above) so that the hot kernel reads them as constants.
+struct __align__(16) RoundKeys {
+    uint32_t k[20];  // k[2r] = key word 0 of round r, k[2r+1] = key word 1
+};
+__host__ __device__ inline RoundKeys expand_keys(uint64_t seed)
+{
+    RoundKeys rk;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        rk.k[2 * r] = k0;
+        rk.k[2 * r + 1] = k1;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    return rk;
+}
+__device__ __forceinline__ Words philox_keyed(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const RoundKeys& rk)
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        c0 = hi1 ^ c1 ^ rk.k[2 * r];
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ rk.k[2 * r + 1];
+        c3 = lo0;
+    }
+    return {c0, c1, c2, c3};
+}
 
 // ---------------------------------------------------------------- per-precision math
 template <typename Real>
 struct M;
 template <>
 struct M<float> {
-    // fp32 rule: u = (2*(w>>9)+1) * 2^-24, exact, strictly inside (0,1)
-    static __device__ __forceinline__ float uniform(uint32_t w)
-    {
-        return (float)(2u * (w >> 9) + 1u) * (1.0f / 16777216.0f);
-    }
+    // fp32 rule: u = (2*(w>>9)+1) * 2^-24, exact, strictly inside (0,1).
+    // Built from the bits: f = 1.m in [1,2) with m = w>>9, then u = f - (1 - 2^-24) (exact).
+    static __device__ __forceinline__ float one_two(uint32_t w) { return __uint_as_float(0x3F800000u | (w >> 9)); }
+    static __device__ __forceinline__ float uniform(uint32_t w) { return one_two(w) - 0.99999994f; }
     static __device__ __forceinline__ float log(float x) { return logf(x); }
     static __device__ __forceinline__ float sqrt(float x) { return sqrtf(x); }
     static __device__ __forceinline__ float rcp(float x) { return 1.0f / x; }
@@ -158,8 +197,44 @@ struct M<float> {
         asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
         return r;
     }
+    static __device__ __forceinline__ float lg2(float x)
+    {
+        float r;
+        asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return r;
+    }
+    // angle 2 pi u - pi in (-pi, pi): (f - 1.5) is exact, one rounding in the FMA
+    static __device__ __forceinline__ float angle(uint32_t w)
+    {
+        return fmaf(one_two(w) - 1.5f, 6.2831855f, 3.7450704e-7f);  // 2 pi (u - 1/2), 2 pi 2^-24
+    }
     static __device__ __forceinline__ float cos2pi(float x) { return cospif(2.0f * x); }
     static __device__ __forceinline__ void sincos2pi(float x, float* s, float* c) { sincospif(2.0f * x, s, c); }
+    // sin, cos of 2 pi u(w) by MUFU on the reduced angle: sin(2 pi u) = -sin(2 pi u - pi)
+    static __device__ __forceinline__ void sincos2pi_word(uint32_t w, float* s, float* c)
+    {
+        const float x = angle(w);
+        *s = -__sinf(x);
+        *c = -__cosf(x);
+    }
+    // [R6] delta of one KP trial, MUFU lg2/cos (abs. error of delta <= ~4e-7/alpha)
+    static __device__ __forceinline__ float kp_delta(const Words& w, float inv_alpha)
+    {
+        const float cs = __cosf(angle(w.w1));  // cos(2 pi R' - pi); only its square is used
+        const float g2 = fmaf(cs * cs, lg2(uniform(w.w2)), lg2(uniform(w.w0)));
+        return g2 * (-0.6931472f * inv_alpha);
+    }
+    // The radius sqrt(delta(2-delta)) amplifies the absolute error of delta by 1/radius:
+    // where that would exceed ~1e-6 (radius^2 < 0.12/alpha^2, probability ~1e-4) the
+    // accepted trial is recomputed with the accurate logf/cospif.
+    static __device__ __forceinline__ float kp_delta_refined(const Words& w, float inv_alpha, float delta)
+    {
+        if (delta * (2.0f - delta) < 0.12f * inv_alpha * inv_alpha) {
+            const float cs = cospif(2.0f * uniform(w.w1));
+            delta = -(logf(uniform(w.w0)) + cs * cs * logf(uniform(w.w2))) * inv_alpha;
+        }
+        return delta;
+    }
     static __device__ __forceinline__ float tiny() { return 1e-20f; }
 };
 template <>
@@ -176,7 +251,32 @@ struct M<double> {
     static __device__ __forceinline__ double sqrt0(double x) { return x * ::rsqrt(fmax(x, 1e-300)); }  // x >= 0
     static __device__ __forceinline__ double cos2pi(double x) { return cospi(2.0 * x); }
     static __device__ __forceinline__ void sincos2pi(double x, double* s, double* c) { sincospi(2.0 * x, s, c); }
+    static __device__ __forceinline__ void sincos2pi_word(uint32_t w, double* s, double* c)
+    {
+        sincospi(2.0 * uniform(w), s, c);
+    }
+    // [R6] delta of one KP trial
+    static __device__ __forceinline__ double kp_delta(const Words& w, double inv_alpha)
+    {
+        const double cs = cospi(2.0 * uniform(w.w1));
+        return -(::log(uniform(w.w0)) + cs * cs * ::log(uniform(w.w2))) * inv_alpha;
+    }
+    static __device__ __forceinline__ double kp_delta_refined(const Words&, double, double delta) { return delta; }
     static __device__ __forceinline__ double tiny() { return 1e-30; }
+};
+
+// per-launch constants of the heat-bath kernels. The array bases are resolved on the
+// host so that a link address is base + 16*(32-bit index): one IMAD.WIDE per load.
+template <typename Real>
+struct __align__(16) HbParams {
+    RoundKeys rk;
+    const typename LinkPtr<Real>::type* same[4];  // U_nu on the parity being updated
+    const typename LinkPtr<Real>::type* oppo[4];  // U_nu on the other parity
+    typename LinkPtr<Real>::type* out;            // U_mu on the parity being updated
+    Real inv_beta;
+    uint32_t sweep;
+    uint32_t tag;  // (parity<<2) | mu
+    int parity;
 };
 
 // [R9] Shoemake: uniform unit quaternion from three uniforms

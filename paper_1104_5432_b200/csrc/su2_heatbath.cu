@@ -33,62 +33,67 @@ __device__ __forceinline__ Nbr neighbours(const Geom& g, const Site& c, int r)
     return d;
 }
 
+// The 18 links of the staple are all requested before the first product: one
+// round trip to L2/HBM per thread instead of one per product.
+// Array bases are uniform 64-bit pointers, element indices 32-bit (h + delta < V/2).
 template <typename Real, int MU>
-__device__ __forceinline__ void heatbath_site(typename LinkPtr<Real>::type* __restrict__ links, const Geom& g,
-                                              int p, const Site& c, Real beta, Real inv_beta, uint64_t seed,
-                                              uint32_t sweep, int* __restrict__ err)
+__device__ __forceinline__ void heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
+                                              int* __restrict__ err)
 {
     typedef typename LinkPtr<Real>::type L;
-    const int r = (c.y + c.z + c.t + p) & 1;
+    const int r = (c.y + c.z + c.t + hp.parity) & 1;
     const int h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
     const Nbr d = neighbours(g, c, r);
-    const size_t vh = g.vh;
-    const L* same = links + (size_t)(p * 4) * vh;        // arrays of parity p
-    const L* oppo = links + (size_t)((1 - p) * 4) * vh;  // arrays of parity 1-p
-    const L* o_mu = oppo + MU * vh;                      // U_mu on the other parity
+    const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
+    const uint32_t h_up = (uint32_t)(h + d.up[MU]);
+
+    Quat<Real> a[3], b[3], cc[3], a2[3], b2[3], c2[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const int nu = i + (i >= MU ? 1 : 0);
+        const L* s_nu = hp.same[nu];
+        const L* o_nu = hp.oppo[nu];
+        const uint32_t h_dn = (uint32_t)(h + d.dn[nu]);
+        a[i] = ldq(o_nu + h_up);                               // U_nu(x+mu)
+        b[i] = ldq(o_mu + (uint32_t)(h + d.up[nu]));           // U_mu(x+nu)
+        cc[i] = ldq(s_nu + (uint32_t)h);                       // U_nu(x)
+        a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));  // U_nu(x+mu-nu)
+        b2[i] = ldq(o_mu + h_dn);                              // U_mu(x-nu)
+        c2[i] = ldq(o_nu + h_dn);                              // U_nu(x-nu)
+    }
+
+    // [R5] counter = (s, sweep, (p<<2)|mu, n); the n = 0 draw does not depend on the links
+    const uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
+    const uint32_t tag = hp.tag;
+    const Words wd = philox_keyed(s, hp.sweep, tag, 0u, hp.rk);
 
     // [R3] staple sum, nu ascending, forward then backward, products left to right;
     // the second product of every term accumulates straight into v (FMA chains).
     Quat<Real> v = {0, 0, 0, 0};
-    const int h_up = h + d.up[MU];
 #pragma unroll
-    for (int nu = 0; nu < 4; ++nu) {
-        if (nu == MU) continue;
-        const L* s_nu = same + nu * vh;
-        const L* o_nu = oppo + nu * vh;
-        const int h_dn = h + d.dn[nu];
-        const Quat<Real> a = ldq(o_nu + h_up);                // U_nu(x+mu)
-        const Quat<Real> b = ldq(o_mu + (h + d.up[nu]));      // U_mu(x+nu)
-        const Quat<Real> cc = ldq(s_nu + h);                  // U_nu(x)
-        const Quat<Real> a2 = ldq(s_nu + (h_up + d.dn[nu]));  // U_nu(x+mu-nu)
-        const Quat<Real> b2 = ldq(o_mu + h_dn);               // U_mu(x-nu)
-        const Quat<Real> c2 = ldq(o_nu + h_dn);               // U_nu(x-nu)
-        qmac<false, true>(v, qmul<false, true>(a, b), cc);    // (a b^+) c^+
-        qmac<false, false>(v, qmul<true, true>(a2, b2), c2);  // (a2^+ b2^+) c2
+    for (int i = 0; i < 3; ++i) {
+        qmac<false, true>(v, qmul<false, true>(a[i], b[i]), cc[i]);    // (a b^+) c^+
+        qmac<false, false>(v, qmul<true, true>(a2[i], b2[i]), c2[i]);  // (a2^+ b2^+) c2
     }
-
-    // [R5] counter = (s, sweep, (p<<2)|mu, n)
-    const uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
-    const uint32_t tag = ((uint32_t)p << 2) | (uint32_t)MU;
-    const Words wd = draw(seed, s, sweep, tag, 0u);
 
     const Real k2 = v.a0 * v.a0 + v.a1 * v.a1 + v.a2 * v.a2 + v.a3 * v.a3;
     Quat<Real> u;
     if (k2 < M<Real>::tiny()) {  // [R8]
         u = haar_from_words<Real>(wd);
     } else {
-        const Real rk = M<Real>::rsqrt(k2);      // 1/k
-        const Real inv_alpha = rk * inv_beta;    // 1/(beta k)
+        const Real rk = M<Real>::rsqrt(k2);       // 1/k
+        const Real inv_alpha = rk * hp.inv_beta;  // 1/(beta k)
         // [R6] Kennedy-Pendleton
         Real delta = 0;
         uint32_t n = 1;
         for (;;) {
-            const Words w = draw(seed, s, sweep, tag, n);
-            const Real R = M<Real>::uniform(w.w0), Rp = M<Real>::uniform(w.w1);
-            const Real Rpp = M<Real>::uniform(w.w2), Rppp = M<Real>::uniform(w.w3);
-            const Real cs = M<Real>::cos2pi(Rp);
-            delta = -(M<Real>::log(R) + cs * cs * M<Real>::log(Rpp)) * inv_alpha;
-            if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) break;
+            const Words w = philox_keyed(s, hp.sweep, tag, n, hp.rk);
+            delta = M<Real>::kp_delta(w, inv_alpha);
+            const Real Rppp = M<Real>::uniform(w.w3);
+            if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) {
+                delta = M<Real>::kp_delta_refined(w, inv_alpha, delta);
+                break;
+            }
             if (++n > 10000u) {  // unreachable for alpha >~ 1e-4; flag, keep x0 = 1
                 atomicOr(err, 1);
                 delta = 0;
@@ -101,22 +106,38 @@ __device__ __forceinline__ void heatbath_site(typename LinkPtr<Real>::type* __re
         const Real cth = (Real)1 - (Real)2 * M<Real>::uniform(wd.w0);
         const Real sth = M<Real>::sqrt0(fmax((Real)1 - cth * cth, (Real)0));
         Real sphi, cphi;
-        M<Real>::sincos2pi(M<Real>::uniform(wd.w1), &sphi, &cphi);
+        M<Real>::sincos2pi_word(wd.w1, &sphi, &cphi);
         const Real rs = rad * sth;
         const Quat<Real> X = {x0, rs * cphi, rs * sphi, rad * cth};
         u = qmul<false, true>(X, v);  // X * v^dagger = k * (X * Vbar^dagger); k drops out below
     }
     const Real inv = M<Real>::rsqrt(u.a0 * u.a0 + u.a1 * u.a1 + u.a2 * u.a2 + u.a3 * u.a3);
     u.a0 *= inv; u.a1 *= inv; u.a2 *= inv; u.a3 *= inv;
-    stq(links + (size_t)(p * 4 + MU) * vh + h, u);
+    stq(hp.out + (uint32_t)h, u);
 }
+
+// Resident CTAs per SM that ptxas must allow: this is the register budget that lets it
+// keep all 18 link loads of a thread in flight at once.
+#ifndef HB_MINB_F32
+#define HB_MINB_F32 8
+#endif
+#ifndef HB_MINB_F64
+#define HB_MINB_F64 8
+#endif
+template <typename Real>
+struct MinBlocks {
+    static constexpr int value = HB_MINB_F32;
+};
+template <>
+struct MinBlocks<double> {
+    static constexpr int value = HB_MINB_F64;
+};
 
 // tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile;
 // grid = (nb0, nb1, nb2*nb3): x fastest, so CTAs are scheduled roughly in memory order.
 template <typename Real, int MU, int LHX, int LY, int LZ, int LT>
-__global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT))
-    heatbath_tiled_kernel(typename LinkPtr<Real>::type* __restrict__ links, const Geom g, int p, Real beta,
-                          Real inv_beta, uint64_t seed, uint32_t sweep, int* __restrict__ err)
+__global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::value)
+    heatbath_tiled_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
     const uint32_t bzt = blockIdx.z;
     const uint32_t bt = (g.nb[2] == 1) ? bzt : __umulhi(bzt, g.zmagic);
@@ -127,14 +148,13 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT))
     c.y = (int)(blockIdx.y << LY) + ((tid >> LHX) & ((1 << LY) - 1));
     c.z = (int)(bz << LZ) + ((tid >> (LHX + LY)) & ((1 << LZ) - 1));
     c.t = (int)(bt << LT) + (tid >> (LHX + LY + LZ));
-    heatbath_site<Real, MU>(links, g, p, c, beta, inv_beta, seed, sweep, err);
+    heatbath_site<Real, MU>(g, c, hp, err);
 }
 
 // linear launch: thread i <-> half-index h = i; any even extents
 template <typename Real, int MU>
 __global__ void __launch_bounds__(kBlock)
-    heatbath_linear_kernel(typename LinkPtr<Real>::type* __restrict__ links, const Geom g, int p, Real beta,
-                           Real inv_beta, uint64_t seed, uint32_t sweep, int* __restrict__ err)
+    heatbath_linear_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
     const uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
     if (h >= g.vh) return;
@@ -145,7 +165,7 @@ __global__ void __launch_bounds__(kBlock)
     c.y = (int)(q - q2 * (uint32_t)g.n[1]);
     c.t = (int)(q2 / (uint32_t)g.n[2]);
     c.z = (int)(q2 - (uint32_t)c.t * (uint32_t)g.n[2]);
-    heatbath_site<Real, MU>(links, g, p, c, beta, inv_beta, seed, sweep, err);
+    heatbath_site<Real, MU>(g, c, hp, err);
 }
 
 // [R9] init: one thread per link of the device layout
@@ -187,15 +207,25 @@ static int launch_substep_t(void* links, const Geom& g, int parity, double beta,
                             int* err, cudaStream_t st)
 {
     typedef typename LinkPtr<Real>::type L;
+    HbParams<Real> hp;
+    hp.inv_beta = (Real)(1.0 / beta);
+    hp.sweep = sweep;
+    hp.rk = expand_keys(seed);
+    hp.tag = ((uint32_t)parity << 2) | (uint32_t)MU;
+    hp.parity = parity;
+    for (int nu = 0; nu < 4; ++nu) {
+        hp.same[nu] = (const L*)links + (size_t)(parity * 4 + nu) * g.vh;
+        hp.oppo[nu] = (const L*)links + (size_t)((1 - parity) * 4 + nu) * g.vh;
+    }
+    hp.out = (L*)links + (size_t)(parity * 4 + MU) * g.vh;
     if (tiled_ok(g)) {
         constexpr int T = 1 << (kTileLog2[0] + kTileLog2[1] + kTileLog2[2] + kTileLog2[3]);
         const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
         heatbath_tiled_kernel<Real, MU, kTileLog2[0], kTileLog2[1], kTileLog2[2], kTileLog2[3]>
-            <<<grid, T, 0, st>>>((L*)links, g, parity, (Real)beta, (Real)(1.0 / beta), seed, sweep, err);
+            <<<grid, T, 0, st>>>(g, hp, err);
     } else {
         const unsigned grid = (g.vh + kBlock - 1) / kBlock;
-        heatbath_linear_kernel<Real, MU><<<grid, kBlock, 0, st>>>((L*)links, g, parity, (Real)beta, (Real)(1.0 / beta), seed,
-                                                                  sweep, err);
+        heatbath_linear_kernel<Real, MU><<<grid, kBlock, 0, st>>>(g, hp, err);
     }
     return 1;
 }

@@ -10,7 +10,13 @@ namespace su2 {
 
 // Tile of one CTA of the tiled heat-bath launch, in threads: (hx, y, z, t).
 // Used when every extent is a multiple of the tile (else the linear launch).
-constexpr int kTileLog2[4] = {3, 2, 2, 1};  // 8 x 4 x 4 x 2 = 256 threads, 16 sites along x
+#ifndef HB_T0
+#define HB_T0 3
+#define HB_T1 2
+#define HB_T2 1
+#define HB_T3 1
+#endif
+constexpr int kTileLog2[4] = {HB_T0, HB_T1, HB_T2, HB_T3};  // 8 x 4 x 2 x 2 = 128 threads, 16 sites along x
 constexpr int kBlock = 256;                 // block size of every other kernel; part of the
                                             // definition of the fixed-order reductions
 
