@@ -2,6 +2,7 @@
 // checking, error capture, stream plumbing. No arithmetic of the method lives here.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -21,6 +22,9 @@ struct su2_lattice {
     bool initialised;
     Scratch sc;
     uint64_t launches;
+    int last_substep;  // 2*mu+parity of the heat-bath sub-step that was the LAST work enqueued by this
+                       // handle, else -1: decides whether the next sub-step may overlap it
+    bool pdl;          // programmatic dependent launch enabled (SU2HB_NO_PDL=1 disables; A/B timing only)
     int sticky;  // sticky error code
     char msg[256];
 };
@@ -46,6 +50,19 @@ static int fail(su2_lattice* lat, int code, const char* what, cudaError_t ce = c
         if (!(lat)) return SU2_EARG;     \
         if ((lat)->sticky) return (lat)->sticky; \
     } while (0)
+// every entry point that enqueues anything other than a heat-bath sub-step
+#define NOT_A_SUBSTEP(lat) ((lat)->last_substep = -1)
+
+// launch sub-step (mu, parity); it may overlap the tail of the previous launch only if
+// that was its canonical predecessor [R4] on this handle
+static void enqueue_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, int mu, int parity)
+{
+    const int idx = 2 * mu + parity;
+    const bool overlap = lat->pdl && lat->last_substep == (idx + 7) % 8;
+    lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, parity, beta, lat->seed,
+                                             sweep_idx, lat->sc.err, overlap, lat->stream);
+    lat->last_substep = idx;
+}
 
 static bool valid_dims(int Nx, int Ny, int Nz, int Nt, int precision)
 {
@@ -84,20 +101,17 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
     g.sz = g.nxh * Ny;
     g.st = g.nxh * Ny * Nz;
     g.vh = (uint32_t)((uint64_t)Nx * Ny * Nz * Nt / 2);
-    g.nb[0] = g.nb[1] = g.nb[2] = g.nb[3] = 0;
     g.wup[0] = -(g.nxh - 1);
     g.wup[1] = -(Ny - 1) * g.sy;
     g.wup[2] = -(Nz - 1) * g.sz;
     g.wup[3] = -(Nt - 1) * g.st;
-    g.zmagic = 0;
-    if (tiled_ok(g)) {
-        g.nb[0] = g.nxh >> kTileLog2[0];
-        g.nb[1] = Ny >> kTileLog2[1];
-        g.nb[2] = Nz >> kTileLog2[2];
-        g.nb[3] = Nt >> kTileLog2[3];
-        g.zmagic = (uint32_t)(((1ull << 32) + (uint64_t)g.nb[2] - 1) / (uint64_t)g.nb[2]);  // unused if nb2 == 1
-    }
+    choose_tiling(g);
     lat->precision = precision;
+    lat->last_substep = -1;
+    {
+        const char* e = getenv("SU2HB_NO_PDL");
+        lat->pdl = !(e && e[0] == '1');
+    }
     lat->stream = (cudaStream_t)stream;
     lat->owns_links = !external;
     lat->links = dev_links;
@@ -147,6 +161,7 @@ extern "C" int su2_lattice_destroy(su2_lattice* lat)
 extern "C" int su2_set_stream(su2_lattice* lat, void* cuda_stream)
 {
     ENTER(lat);
+    NOT_A_SUBSTEP(lat);
     lat->stream = (cudaStream_t)cuda_stream;
     return SU2_OK;
 }
@@ -154,6 +169,7 @@ extern "C" int su2_set_stream(su2_lattice* lat, void* cuda_stream)
 extern "C" int su2_init(su2_lattice* lat, int start, uint64_t seed)
 {
     ENTER(lat);
+    NOT_A_SUBSTEP(lat);
     if (start != SU2_START_COLD && start != SU2_START_HOT) return fail(lat, SU2_EARG, "su2_init: bad start");
     lat->launches += launch_init(lat->links, lat->g, lat->precision, start, seed, lat->stream);
     CK(lat, cudaGetLastError());
@@ -181,8 +197,7 @@ extern "C" int su2_heatbath_substep(su2_lattice* lat, double beta, uint32_t swee
     ENTER(lat);
     if (int rc = check_beta(lat, beta)) return rc;
     if (mu < 0 || mu > 3 || (parity != 0 && parity != 1)) return fail(lat, SU2_EARG, "bad mu / parity");
-    lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, parity, beta, lat->seed,
-                                             sweep_idx, lat->sc.err, lat->stream);
+    enqueue_substep(lat, beta, sweep_idx, mu, parity);
     CK(lat, cudaGetLastError());
     return SU2_OK;
 }
@@ -192,10 +207,8 @@ extern "C" int su2_heatbath_sweep(su2_lattice* lat, double beta, uint32_t sweep_
     ENTER(lat);
     if (int rc = check_beta(lat, beta)) return rc;
     for (int mu = 0; mu < 4; ++mu)      // [R4] direction outer,
-        for (int p = 0; p < 2; ++p) {   //      parity inner
-            lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, p, beta, lat->seed,
-                                                     sweep_idx, lat->sc.err, lat->stream);
-        }
+        for (int p = 0; p < 2; ++p)     //      parity inner
+            enqueue_substep(lat, beta, sweep_idx, mu, p);
     CK(lat, cudaGetLastError());
     return SU2_OK;
 }
@@ -213,12 +226,14 @@ static int sync_and_check(su2_lattice* lat)
 extern "C" int su2_synchronize(su2_lattice* lat)
 {
     ENTER(lat);
+    NOT_A_SUBSTEP(lat);
     return sync_and_check(lat);
 }
 
 extern "C" int su2_measure_async(su2_lattice* lat, double* dev_out, size_t index)
 {
     ENTER(lat);
+    NOT_A_SUBSTEP(lat);
     if (!dev_out) return fail(lat, SU2_EARG, "su2_measure_async: NULL dev_out");
     if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
     lat->launches += launch_plaquette(lat->links, lat->g, lat->precision, lat->sc, dev_out + 2 * index, lat->stream);
@@ -231,6 +246,7 @@ extern "C" int su2_measure_async(su2_lattice* lat, double* dev_out, size_t index
 extern "C" int su2_measure(su2_lattice* lat, double* plaquette_out, double* polyakov_out)
 {
     ENTER(lat);
+    NOT_A_SUBSTEP(lat);
     if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
     if (plaquette_out)
         lat->launches += launch_plaquette(lat->links, lat->g, lat->precision, lat->sc, lat->sc.out, lat->stream);
@@ -260,6 +276,7 @@ extern "C" int su2_polyakov_loop(su2_lattice* lat, double* out)
 extern "C" int su2_polyakov_correlator(su2_lattice* lat, int rmax, double* out)
 {
     ENTER(lat);
+    NOT_A_SUBSTEP(lat);
     if (!out) return fail(lat, SU2_EARG, "NULL out");
     if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
     int nmin = lat->g.n[0] < lat->g.n[1] ? lat->g.n[0] : lat->g.n[1];
@@ -275,6 +292,7 @@ extern "C" int su2_polyakov_correlator(su2_lattice* lat, int rmax, double* out)
 extern "C" int su2_get_links(su2_lattice* lat, void* host_dst, size_t bytes)
 {
     ENTER(lat);
+    NOT_A_SUBSTEP(lat);
     const Geom& g = lat->g;
     const size_t need = su2_lattice_bytes(g.n[0], g.n[1], g.n[2], g.n[3], lat->precision);
     if (!host_dst || bytes != need) return fail(lat, SU2_EARG, "su2_get_links: bad buffer");
@@ -296,6 +314,7 @@ extern "C" int su2_get_links(su2_lattice* lat, void* host_dst, size_t bytes)
 extern "C" int su2_set_links(su2_lattice* lat, const void* host_src, size_t bytes)
 {
     ENTER(lat);
+    NOT_A_SUBSTEP(lat);
     const Geom& g = lat->g;
     const size_t need = su2_lattice_bytes(g.n[0], g.n[1], g.n[2], g.n[3], lat->precision);
     if (!host_src || bytes != need) return fail(lat, SU2_EARG, "su2_set_links: bad buffer");

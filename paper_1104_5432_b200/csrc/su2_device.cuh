@@ -18,10 +18,51 @@ struct Geom {
     int nxh;         // Nx/2
     int sy, sz, st;  // strides of y, z, t in half-index units: nxh, nxh*Ny, nxh*Ny*Nz
     uint32_t vh;     // V/2
+    int tile;        // tiled launch: which tile shape (su2_launch.h kTiles), -1 = linear launch
     int nb[4];       // tiled launch: number of tiles along hx, y, z, t
     int wup[4];      // half-index delta of +mu at the upper boundary: -(N-1)*stride  (x: -(nxh-1))
     uint32_t zmagic; // ceil(2^32 / nb[2]): blockIdx.z -> (bz, bt) without a division
 };
+
+// ---------------------------------------------------------------- sites and neighbours
+struct Site {
+    int hx, y, z, t;  // hx = x>>1
+};
+
+// half-index deltas of the 8 neighbours; r = low bit of x
+struct Nbr {
+    int up[4], dn[4];
+};
+__device__ __forceinline__ Nbr neighbours(const Geom& g, const Site& c, int r)
+{
+    Nbr d;
+    d.up[0] = r ? ((c.hx + 1 == g.nxh) ? g.wup[0] : 1) : 0;
+    d.dn[0] = r ? 0 : ((c.hx == 0) ? -g.wup[0] : -1);
+    d.up[1] = (c.y + 1 == g.n[1]) ? g.wup[1] : g.sy;
+    d.dn[1] = (c.y == 0) ? -g.wup[1] : -g.sy;
+    d.up[2] = (c.z + 1 == g.n[2]) ? g.wup[2] : g.sz;
+    d.dn[2] = (c.z == 0) ? -g.wup[2] : -g.sz;
+    d.up[3] = (c.t + 1 == g.n[3]) ? g.wup[3] : g.st;
+    d.dn[3] = (c.t == 0) ? -g.wup[3] : -g.st;
+    return d;
+}
+
+// Tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile; grid =
+// (nb0, nb1, nb2*nb3[*k]), x fastest, so CTAs are scheduled roughly in memory order.
+// `bzt` = bz + nb2*bt (blockIdx.z, or blockIdx.z with extra factors divided out).
+template <int LHX, int LY, int LZ, int LT>
+__device__ __forceinline__ Site tile_site(const Geom& g, uint32_t bzt)
+{
+    const uint32_t bt = (g.nb[2] == 1) ? bzt : __umulhi(bzt, g.zmagic);
+    const uint32_t bz = bzt - bt * (uint32_t)g.nb[2];
+    const int tid = threadIdx.x;
+    Site c;
+    c.hx = (int)(blockIdx.x << LHX) + (tid & ((1 << LHX) - 1));
+    c.y = (int)(blockIdx.y << LY) + ((tid >> LHX) & ((1 << LY) - 1));
+    c.z = (int)(bz << LZ) + ((tid >> (LHX + LY)) & ((1 << LZ) - 1));
+    c.t = (int)(bt << LT) + (tid >> (LHX + LY + LZ));
+    return c;
+}
 
 // ---------------------------------------------------------------- quaternions
 template <typename Real>
@@ -67,6 +108,31 @@ __device__ __forceinline__ Quat<double> ldq(const double4a* p)
 #ifndef HB_ST
 #define HB_ST ".cs"
 #endif
+// L2-only loads (no L1 allocation): used for the links the preceding sub-step wrote,
+// which are read after griddepcontrol.wait while that kernel may still share the SM.
+__device__ __forceinline__ Quat<float> ldq_cg(const float4* p)
+{
+    Quat<float> q;
+    asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(q.a0), "=f"(q.a1), "=f"(q.a2), "=f"(q.a3)
+                 : "l"(p)
+                 : "memory");
+    return q;
+}
+__device__ __forceinline__ Quat<double> ldq_cg(const double4a* p)
+{
+    Quat<double> q;
+    asm volatile("ld.global.cg.v4.f64 {%0,%1,%2,%3}, [%4];"
+                 : "=d"(q.a0), "=d"(q.a1), "=d"(q.a2), "=d"(q.a3)
+                 : "l"(p)
+                 : "memory");
+    return q;
+}
+// Programmatic dependent launch: wait for the preceding kernel of the
+// stream to finish and flush; then allow the next kernel's CTAs to be scheduled.
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ void stq(float4* p, const Quat<float>& q)
 {
     asm volatile("st.global" HB_ST ".v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(q.a0), "f"(q.a1), "f"(q.a2), "f"(q.a3)
@@ -275,8 +341,6 @@ struct __align__(16) HbParams {
     typename LinkPtr<Real>::type* out;            // U_mu on the parity being updated
     Real inv_beta;
     uint32_t sweep;
-    uint32_t tag;  // (parity<<2) | mu
-    int parity;
 };
 
 // [R9] Shoemake: uniform unit quaternion from three uniforms

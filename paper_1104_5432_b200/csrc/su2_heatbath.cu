@@ -11,41 +11,35 @@
 
 namespace su2 {
 
-struct Site {
-    int hx, y, z, t;  // hx = x>>1
-};
-
-// half-index deltas of the 8 neighbours; r = low bit of x
-struct Nbr {
-    int up[4], dn[4];
-};
-__device__ __forceinline__ Nbr neighbours(const Geom& g, const Site& c, int r)
-{
-    Nbr d;
-    d.up[0] = r ? ((c.hx + 1 == g.nxh) ? g.wup[0] : 1) : 0;
-    d.dn[0] = r ? 0 : ((c.hx == 0) ? -g.wup[0] : -1);
-    d.up[1] = (c.y + 1 == g.n[1]) ? g.wup[1] : g.sy;
-    d.dn[1] = (c.y == 0) ? -g.wup[1] : -g.sy;
-    d.up[2] = (c.z + 1 == g.n[2]) ? g.wup[2] : g.sz;
-    d.dn[2] = (c.z == 0) ? -g.wup[2] : -g.sz;
-    d.up[3] = (c.t + 1 == g.n[3]) ? g.wup[3] : g.st;
-    d.dn[3] = (c.t == 0) ? -g.wup[3] : -g.st;
-    return d;
-}
-
 // The 18 links of the staple are all requested before the first product: one
 // round trip to L2/HBM per thread instead of one per product.
 // Array bases are uniform 64-bit pointers, element indices 32-bit (h + delta < V/2).
-template <typename Real, int MU>
+//
+// Overlap with the preceding sub-step. In the canonical order [R4] the
+// kernel before (MU,P) wrote exactly one array that this one reads:
+//   P = 1: U_MU on parity 0        = hp.oppo[MU]            (the b, b2 loads)
+//   P = 0: U_{MU-1} on parity 1    = hp.oppo[(MU+3)%4]      (the a, c2 loads of that nu)
+// With programmatic dependent launch the CTA is scheduled, decodes its site and computes
+// its neighbour indices in the predecessor's tail, then waits (griddepcontrol.wait) before
+// its first load; loads issued ahead of the wait were measured to cost more (an extra
+// dependent round trip, or spills) than they hide. The predecessor's output is read
+// through L2 (ld.global.cg): its lines may not be taken from an L1 that an overlapping
+// launch did not invalidate. Launched without the attribute the wait is a no-op.
+template <typename Real, int MU, int P>
 __device__ __forceinline__ void heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
                                               int* __restrict__ err)
 {
     typedef typename LinkPtr<Real>::type L;
-    const int r = (c.y + c.z + c.t + hp.parity) & 1;
+    constexpr int DEP_NU = (P == 0) ? (MU + 3) % 4 : -1;
+    constexpr bool DEP_MU = (P == 1);
+    const int r = (c.y + c.z + c.t + P) & 1;
     const int h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
     const Nbr d = neighbours(g, c, r);
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
     const uint32_t h_up = (uint32_t)(h + d.up[MU]);
+
+    grid_dep_wait();    // the preceding kernel of the stream has finished and flushed
+    grid_dep_launch();  // ... so the next one may be scheduled behind this CTA
 
     Quat<Real> a[3], b[3], cc[3], a2[3], b2[3], c2[3];
 #pragma unroll
@@ -54,17 +48,18 @@ __device__ __forceinline__ void heatbath_site(const Geom& g, const Site& c, cons
         const L* s_nu = hp.same[nu];
         const L* o_nu = hp.oppo[nu];
         const uint32_t h_dn = (uint32_t)(h + d.dn[nu]);
-        a[i] = ldq(o_nu + h_up);                               // U_nu(x+mu)
-        b[i] = ldq(o_mu + (uint32_t)(h + d.up[nu]));           // U_mu(x+nu)
-        cc[i] = ldq(s_nu + (uint32_t)h);                       // U_nu(x)
-        a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));  // U_nu(x+mu-nu)
-        b2[i] = ldq(o_mu + h_dn);                              // U_mu(x-nu)
-        c2[i] = ldq(o_nu + h_dn);                              // U_nu(x-nu)
+        const uint32_t h_upnu = (uint32_t)(h + d.up[nu]);
+        a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
+        b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
+        cc[i] = ldq(s_nu + (uint32_t)h);                                  // U_nu(x)
+        a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));             // U_nu(x+mu-nu)
+        b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
+        c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
     }
 
     // [R5] counter = (s, sweep, (p<<2)|mu, n); the n = 0 draw does not depend on the links
     const uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
-    const uint32_t tag = hp.tag;
+    const uint32_t tag = ((uint32_t)P << 2) | (uint32_t)MU;
     const Words wd = philox_keyed(s, hp.sweep, tag, 0u, hp.rk);
 
     // [R3] staple sum, nu ascending, forward then backward, products left to right;
@@ -135,24 +130,16 @@ struct MinBlocks<double> {
 
 // tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile;
 // grid = (nb0, nb1, nb2*nb3): x fastest, so CTAs are scheduled roughly in memory order.
-template <typename Real, int MU, int LHX, int LY, int LZ, int LT>
+template <typename Real, int MU, int P, int LHX, int LY, int LZ, int LT>
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::value)
     heatbath_tiled_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
-    const uint32_t bzt = blockIdx.z;
-    const uint32_t bt = (g.nb[2] == 1) ? bzt : __umulhi(bzt, g.zmagic);
-    const uint32_t bz = bzt - bt * (uint32_t)g.nb[2];
-    const int tid = threadIdx.x;
-    Site c;
-    c.hx = (int)(blockIdx.x << LHX) + (tid & ((1 << LHX) - 1));
-    c.y = (int)(blockIdx.y << LY) + ((tid >> LHX) & ((1 << LY) - 1));
-    c.z = (int)(bz << LZ) + ((tid >> (LHX + LY)) & ((1 << LZ) - 1));
-    c.t = (int)(bt << LT) + (tid >> (LHX + LY + LZ));
-    heatbath_site<Real, MU>(g, c, hp, err);
+    const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z);
+    heatbath_site<Real, MU, P>(g, c, hp, err);
 }
 
 // linear launch: thread i <-> half-index h = i; any even extents
-template <typename Real, int MU>
+template <typename Real, int MU, int P>
 __global__ void __launch_bounds__(kBlock)
     heatbath_linear_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
@@ -165,7 +152,7 @@ __global__ void __launch_bounds__(kBlock)
     c.y = (int)(q - q2 * (uint32_t)g.n[1]);
     c.t = (int)(q2 / (uint32_t)g.n[2]);
     c.z = (int)(q2 - (uint32_t)c.t * (uint32_t)g.n[2]);
-    heatbath_site<Real, MU>(g, c, hp, err);
+    heatbath_site<Real, MU, P>(g, c, hp, err);
 }
 
 // [R9] init: one thread per link of the device layout
@@ -192,61 +179,99 @@ __global__ void __launch_bounds__(kBlock)
     stq(links + (size_t)arr * g.vh + h, u);
 }
 
-bool tiled_ok(const Geom& g)
+void choose_tiling(Geom& g)
 {
-    // grid limits (y, z <= 65535) and exactness of the zmagic split: nb2^2 * nb3 < 2^32
-    const uint64_t t0 = g.nxh >> kTileLog2[0], t1 = g.n[1] >> kTileLog2[1], t2 = g.n[2] >> kTileLog2[2],
-                   t3 = g.n[3] >> kTileLog2[3];
-    if (t1 > 65535 || t2 * t3 > 65535 || t0 == 0) return false;
-    return g.nxh % (1 << kTileLog2[0]) == 0 && g.n[1] % (1 << kTileLog2[1]) == 0 &&
-           g.n[2] % (1 << kTileLog2[2]) == 0 && g.n[3] % (1 << kTileLog2[3]) == 0;
+    g.tile = -1;
+    g.nb[0] = g.nb[1] = g.nb[2] = g.nb[3] = 0;
+    g.zmagic = 0;
+    for (int k = 0; k < kNumTiles; ++k) {
+        const int* t = kTiles[k];
+        const int ext[4] = {g.nxh, g.n[1], g.n[2], g.n[3]};
+        bool ok = true;
+        for (int d = 0; d < 4; ++d) ok = ok && ext[d] % (1 << t[d]) == 0;
+        if (!ok) continue;
+        const uint64_t nb1 = g.n[1] >> t[1], nb2 = g.n[2] >> t[2], nb3 = g.n[3] >> t[3];
+        // grid limits (y, z <= 65535) and exactness of the zmagic split: nb2^2 * nb3 < 2^32
+        if (nb1 > 65535 || nb2 * nb3 > 65535) continue;
+        g.tile = k;
+        g.nb[0] = g.nxh >> t[0];
+        g.nb[1] = (int)nb1;
+        g.nb[2] = (int)nb2;
+        g.nb[3] = (int)nb3;
+        g.zmagic = (uint32_t)(((1ull << 32) + nb2 - 1) / nb2);  // unused if nb2 == 1
+        return;
+    }
 }
 
-template <typename Real, int MU>
-static int launch_substep_t(void* links, const Geom& g, int parity, double beta, uint64_t seed, uint32_t sweep,
-                            int* err, cudaStream_t st)
+// One launch through cudaLaunchKernelEx; `overlap` adds the programmatic-stream-
+// serialization attribute (the kernel may start while its predecessor drains).
+template <typename... KArgs, typename... Args>
+static void launch_ex(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, bool overlap, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = overlap ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
+template <typename Real, int MU, int P>
+static int launch_substep_t(void* links, const Geom& g, double beta, uint64_t seed, uint32_t sweep, int* err,
+                            bool overlap, cudaStream_t st)
 {
     typedef typename LinkPtr<Real>::type L;
     HbParams<Real> hp;
     hp.inv_beta = (Real)(1.0 / beta);
     hp.sweep = sweep;
     hp.rk = expand_keys(seed);
-    hp.tag = ((uint32_t)parity << 2) | (uint32_t)MU;
-    hp.parity = parity;
     for (int nu = 0; nu < 4; ++nu) {
-        hp.same[nu] = (const L*)links + (size_t)(parity * 4 + nu) * g.vh;
-        hp.oppo[nu] = (const L*)links + (size_t)((1 - parity) * 4 + nu) * g.vh;
+        hp.same[nu] = (const L*)links + (size_t)(P * 4 + nu) * g.vh;
+        hp.oppo[nu] = (const L*)links + (size_t)((1 - P) * 4 + nu) * g.vh;
     }
-    hp.out = (L*)links + (size_t)(parity * 4 + MU) * g.vh;
-    if (tiled_ok(g)) {
-        constexpr int T = 1 << (kTileLog2[0] + kTileLog2[1] + kTileLog2[2] + kTileLog2[3]);
-        const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
-        heatbath_tiled_kernel<Real, MU, kTileLog2[0], kTileLog2[1], kTileLog2[2], kTileLog2[3]>
-            <<<grid, T, 0, st>>>(g, hp, err);
+    hp.out = (L*)links + (size_t)(P * 4 + MU) * g.vh;
+    const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
+    if (g.tile == 0) {
+        launch_ex(heatbath_tiled_kernel<Real, MU, P, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>, grid,
+                  dim3(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3])), st, overlap, g, hp, err);
+    } else if (g.tile == 1) {
+        launch_ex(heatbath_tiled_kernel<Real, MU, P, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3]>, grid,
+                  dim3(1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3])), st, overlap, g, hp, err);
     } else {
-        const unsigned grid = (g.vh + kBlock - 1) / kBlock;
-        heatbath_linear_kernel<Real, MU><<<grid, kBlock, 0, st>>>(g, hp, err);
+        const unsigned nblk = (g.vh + kBlock - 1) / kBlock;
+        launch_ex(heatbath_linear_kernel<Real, MU, P>, dim3(nblk), dim3(kBlock), st, overlap, g, hp, err);
     }
     return 1;
 }
 
 template <typename Real>
 static int launch_substep_p(void* links, const Geom& g, int mu, int parity, double beta, uint64_t seed,
-                            uint32_t sweep, int* err, cudaStream_t st)
+                            uint32_t sweep, int* err, bool overlap, cudaStream_t st)
 {
-    switch (mu) {
-        case 0: return launch_substep_t<Real, 0>(links, g, parity, beta, seed, sweep, err, st);
-        case 1: return launch_substep_t<Real, 1>(links, g, parity, beta, seed, sweep, err, st);
-        case 2: return launch_substep_t<Real, 2>(links, g, parity, beta, seed, sweep, err, st);
-        default: return launch_substep_t<Real, 3>(links, g, parity, beta, seed, sweep, err, st);
+    switch (mu * 2 + parity) {
+        case 0: return launch_substep_t<Real, 0, 0>(links, g, beta, seed, sweep, err, overlap, st);
+        case 1: return launch_substep_t<Real, 0, 1>(links, g, beta, seed, sweep, err, overlap, st);
+        case 2: return launch_substep_t<Real, 1, 0>(links, g, beta, seed, sweep, err, overlap, st);
+        case 3: return launch_substep_t<Real, 1, 1>(links, g, beta, seed, sweep, err, overlap, st);
+        case 4: return launch_substep_t<Real, 2, 0>(links, g, beta, seed, sweep, err, overlap, st);
+        case 5: return launch_substep_t<Real, 2, 1>(links, g, beta, seed, sweep, err, overlap, st);
+        case 6: return launch_substep_t<Real, 3, 0>(links, g, beta, seed, sweep, err, overlap, st);
+        default: return launch_substep_t<Real, 3, 1>(links, g, beta, seed, sweep, err, overlap, st);
     }
 }
 
+// `overlap` may be true only if the launch before this one on `st` was the canonical
+// predecessor sub-step [R4] of the same lattice (see heatbath_site).
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
-                            uint64_t seed, uint32_t sweep, int* err, cudaStream_t st)
+                            uint64_t seed, uint32_t sweep, int* err, bool overlap, cudaStream_t st)
 {
-    return precision == 32 ? launch_substep_p<float>(links, g, mu, parity, beta, seed, sweep, err, st)
-                           : launch_substep_p<double>(links, g, mu, parity, beta, seed, sweep, err, st);
+    return precision == 32 ? launch_substep_p<float>(links, g, mu, parity, beta, seed, sweep, err, overlap, st)
+                           : launch_substep_p<double>(links, g, mu, parity, beta, seed, sweep, err, overlap, st);
 }
 
 int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st)

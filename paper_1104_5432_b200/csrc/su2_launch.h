@@ -8,15 +8,18 @@
 
 namespace su2 {
 
-// Tile of one CTA of the tiled heat-bath launch, in threads: (hx, y, z, t).
-// Used when every extent is a multiple of the tile (else the linear launch).
+// Tiles of one CTA of the tiled heat-bath launch, log2 threads along (hx, y, z, t); 128
+// threads each. The first shape whose extents divide the lattice is used, else the
+// linear launch (shapes chosen by measurement, profiles/r01b.md).
 #ifndef HB_T0
-#define HB_T0 3
+#define HB_T0 4
 #define HB_T1 2
 #define HB_T2 1
-#define HB_T3 1
+#define HB_T3 0
 #endif
-constexpr int kTileLog2[4] = {HB_T0, HB_T1, HB_T2, HB_T3};  // 8 x 4 x 2 x 2 = 128 threads, 16 sites along x
+constexpr int kNumTiles = 2;
+constexpr int kTiles[kNumTiles][4] = {{HB_T0, HB_T1, HB_T2, HB_T3},  // 16 x 4 x 2 x 1 (32 sites along x)
+                                      {3, 2, 1, 1}};                  //  8 x 4 x 2 x 2 (16 sites along x)
 constexpr int kBlock = 256;                 // block size of every other kernel; part of the
                                             // definition of the fixed-order reductions
 
@@ -29,13 +32,14 @@ struct Scratch {
 };
 constexpr int kMaxR = 128;
 
-bool tiled_ok(const Geom& g);
+// fills g.tile (index into kTiles or -1), g.nb and g.zmagic
+void choose_tiling(Geom& g);
 size_t partials_needed(const Geom& g);
 
 // each returns the number of kernels it enqueued (0 on launch failure; check cudaGetLastError)
 int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st);
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
-                            uint64_t seed, uint32_t sweep, int* err, cudaStream_t st);
+                            uint64_t seed, uint32_t sweep, int* err, bool overlap, cudaStream_t st);
 int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
                      cudaStream_t st);
 int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,

@@ -55,6 +55,61 @@ __global__ void __launch_bounds__(kBlock)
     if (threadIdx.x == 0) partials[blockIdx.y * gridDim.x + blockIdx.x] = tot;
 }
 
+// Tiled form (same CTA tiles as the heat-bath kernel): grid.z carries
+// (bz, bt, parity), parity slowest. All 16 links of a site are requested before the
+// first product; one partial per CTA, indexed by the linear CTA id.
+#ifndef PLAQ_MINB_F32
+#define PLAQ_MINB_F32 8
+#endif
+#ifndef PLAQ_MINB_F64
+#define PLAQ_MINB_F64 4
+#endif
+template <typename Real, int LHX, int LY, int LZ, int LT>
+__global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), sizeof(Real) == 4 ? PLAQ_MINB_F32 : PLAQ_MINB_F64)
+    plaquette_tiled_kernel(const typename LinkPtr<Real>::type* __restrict__ links, const Geom g,
+                           double* __restrict__ partials)
+{
+    typedef typename LinkPtr<Real>::type L;
+    __shared__ double red[kBlock / 32];
+    const uint32_t nzt = (uint32_t)(g.nb[2] * g.nb[3]);
+    const int p = blockIdx.z >= nzt ? 1 : 0;
+    const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z - (p ? nzt : 0u));
+    const int r = (c.y + c.z + c.t + p) & 1;
+    const int h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
+    int up[4];
+    up[0] = r ? ((c.hx + 1 == g.nxh) ? g.wup[0] : 1) : 0;
+    up[1] = (c.y + 1 == g.n[1]) ? g.wup[1] : g.sy;
+    up[2] = (c.z + 1 == g.n[2]) ? g.wup[2] : g.sz;
+    up[3] = (c.t + 1 == g.n[3]) ? g.wup[3] : g.st;
+    const size_t vh = g.vh;
+    const L* same = links + (size_t)(p * 4) * vh;
+    const L* oppo = links + (size_t)((1 - p) * 4) * vh;
+    Quat<Real> u[4], n1[6], n2[6];
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) u[mu] = ldq(same + mu * vh + (uint32_t)h);
+    {
+        int k = 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu)
+#pragma unroll
+            for (int nu = mu + 1; nu < 4; ++nu, ++k) {
+                n1[k] = ldq(oppo + nu * vh + (uint32_t)(h + up[mu]));  // U_nu(x+mu)
+                n2[k] = ldq(oppo + mu * vh + (uint32_t)(h + up[nu]));  // U_mu(x+nu)
+            }
+    }
+    double acc = 0.0;
+    {
+        int k = 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu)
+#pragma unroll
+            for (int nu = mu + 1; nu < 4; ++nu, ++k)
+                acc += (double)qdot(qmul<false, false>(u[mu], n1[k]), qmul<false, false>(u[nu], n2[k]));
+    }
+    const double tot = block_sum(acc, red);
+    if (threadIdx.x == 0) partials[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = tot;
+}
+
 // final stage: dst[0] = scale * sum(partials[0..n)), fixed order
 __global__ void __launch_bounds__(1024) final_sum_kernel(const double* __restrict__ partials, size_t n, double scale,
                                                          double* __restrict__ dst)
@@ -163,20 +218,48 @@ size_t partials_needed(const Geom& g)
 {
     const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
     size_t a = 2 * (size_t)blocks_for(g.vh);
+    if (g.tile >= 0) {  // one partial per 128-thread tile and parity
+        const size_t t = 2 * (size_t)g.nb[0] * g.nb[1] * g.nb[2] * g.nb[3];
+        if (t > a) a = t;
+    }
     size_t b = (size_t)kMaxR * blocks_for(v3);
     return a > b ? a : b;
+}
+
+template <typename Real>
+static void launch_plaquette_t(const void* links, const Geom& g, const Scratch& sc, size_t* n_partials,
+                               cudaStream_t st)
+{
+    typedef typename LinkPtr<Real>::type L;
+    const uint64_t nz = 2ull * (uint64_t)g.nb[2] * (uint64_t)g.nb[3];
+    if (g.tile >= 0 && nz <= 65535) {
+        const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)nz);
+        *n_partials = (size_t)grid.x * grid.y * grid.z;
+        if (g.tile == 0)
+            plaquette_tiled_kernel<Real, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>
+                <<<grid, 1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3]), 0, st>>>((const L*)links, g,
+                                                                                                    sc.partials);
+        else
+            plaquette_tiled_kernel<Real, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3]>
+                <<<grid, 1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3]), 0, st>>>((const L*)links, g,
+                                                                                                    sc.partials);
+    } else {
+        const dim3 grid(blocks_for(g.vh), 2);
+        *n_partials = (size_t)grid.x * 2;
+        plaquette_kernel<Real><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.partials);
+    }
 }
 
 int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
                      cudaStream_t st)
 {
-    const dim3 grid(blocks_for(g.vh), 2);
+    size_t n = 0;
     if (precision == 32)
-        plaquette_kernel<float><<<grid, kBlock, 0, st>>>((const float4*)links, g, sc.partials);
+        launch_plaquette_t<float>(links, g, sc, &n, st);
     else
-        plaquette_kernel<double><<<grid, kBlock, 0, st>>>((const double4a*)links, g, sc.partials);
+        launch_plaquette_t<double>(links, g, sc, &n, st);
     const double scale = 1.0 / (6.0 * 2.0 * (double)g.vh);
-    final_sum_kernel<<<1, 1024, 0, st>>>(sc.partials, (size_t)grid.x * 2, scale, dev_dst);
+    final_sum_kernel<<<1, 1024, 0, st>>>(sc.partials, n, scale, dev_dst);
     return 2;
 }
 
