@@ -51,34 +51,84 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks/throttle reasons sampled DURING the timed region."""
+    """SM clock, power and throttle reasons sampled DURING the timed region: NVML in a
+    background thread every 10 ms (nvidia-smi -lms as fallback if pynvml is unusable)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
     def __init__(self, index):
         self.index = index
-        self.rows = []
+        self.rows = []  # (time, sm_mhz, sm_max_mhz, power_w, [reasons])
         self.proc = None
+        self.stop_flag = False
+        self.thread = None
+        self.source = None
 
     def start(self):
         try:
+            import pynvml
+            pynvml.nvmlInit()
+            # NVML indexes physical devices: honour CUDA_VISIBLE_DEVICES if it is a list of indices
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            idx = self.index
+            if vis:
+                try:
+                    idx = int(vis.split(",")[self.index])
+                except Exception:
+                    idx = self.index
+            h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            smax = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            bits = [(pynvml.nvmlClocksEventReasonHwSlowdown, "hw_slowdown"),
+                    (pynvml.nvmlClocksEventReasonHwThermalSlowdown, "hw_thermal_slowdown"),
+                    (pynvml.nvmlClocksEventReasonSwThermalSlowdown, "sw_thermal_slowdown"),
+                    (pynvml.nvmlClocksEventReasonSwPowerCap, "sw_power_cap")]
+
+            def loop():
+                while not self.stop_flag:
+                    try:
+                        mhz = float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                        mask = pynvml.nvmlDeviceGetCurrentClocksEventReasons(h)
+                        pw = pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0
+                        self.rows.append((time.time(), mhz, smax, pw, [n for b, n in bits if mask & b]))
+                    except Exception:
+                        pass
+                    time.sleep(0.01)
+
+            self.thread = threading.Thread(target=loop, daemon=True)
+            self.thread.start()
+            self.source = "nvml"
+            return
+        except Exception:
+            pass
+        try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
+            self.source = "nvidia-smi"
         except Exception:
             self.proc = None
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append((time.time(), line.strip()))
+            f = [x.strip() for x in line.split(",")]
+            try:
+                self.rows.append((time.time(), float(f[0]), float(f[1]), float(f[2]),
+                                  [n for n, v in zip(self.NAMES, f[3:7]) if v.lower().startswith("active")]))
+            except Exception:
+                continue
+
+    def ready(self):
+        return bool(self.rows)
 
     def mark(self):
         return time.time()
 
     def stop(self):
+        self.stop_flag = True
         if self.proc:
             self.proc.terminate()
             try:
@@ -87,23 +137,15 @@ class ClockSampler:
                 self.proc.kill()
 
     def summary(self, t0, t1):
-        sm, smax, reasons = [], 0.0, set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for t, line in self.rows:
-            if t < t0 or t > t1 + 0.15:
-                continue
-            f = [x.strip() for x in line.split(",")]
-            try:
-                sm.append(float(f[0]))
-                smax = max(smax, float(f[1]))
-                for n, v in zip(names, f[3:7]):
-                    if v.lower().startswith("active"):
-                        reasons.add(n)
-            except Exception:
-                continue
-        if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": smax, "reasons": sorted(reasons), "samples": len(sm)}
+        rows = [r for r in self.rows if t0 <= r[0] <= t1]
+        if not rows:  # region shorter than one sampling period: nearest samples around it
+            rows = [r for r in self.rows if t0 - 0.1 <= r[0] <= t1 + 0.1]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "source": self.source}
+        reasons = sorted({n for r in rows for n in r[4]})
+        return {"sm_mhz": float(np.median([r[1] for r in rows])), "sm_max_mhz": max(r[2] for r in rows),
+                "power_w": float(np.median([r[3] for r in rows])), "reasons": reasons, "samples": len(rows),
+                "source": self.source}
 
 
 def dist_env():
@@ -251,7 +293,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C5_64^4")
@@ -287,7 +329,7 @@ def main():
     sampler = ClockSampler(local)
     sampler.start()
     t_wait = time.time()
-    while not sampler.rows and time.time() - t_wait < 5.0:  # nvidia-smi takes ~1 s to emit its first line
+    while not sampler.ready() and time.time() - t_wait < 5.0:  # nvidia-smi takes ~1 s to emit its first line
         time.sleep(0.05)
     r = time_workload(pkg, torch, w, prec, args.beta, args.steps, args.warmup, args.seed + rank, sampler, dist)
     clocks = sampler.summary(*r["t_wall"])
@@ -308,11 +350,17 @@ def main():
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": None, "peak_source": peak_src, "kernel": "heatbath sub-step (one per (mu,parity))",
                 "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_us": sub_s * 1e6}
-    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    # traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of that kernel from the
+    # committed `ncu --set full` capture (profiles/traffic.csv: key,bytes_per_launch,source)
+    prof = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(prof):
         try:
             with open(prof) as f:
-                roofline["traffic"] = json.load(f).get(f"{w.name}_fp{prec}")
+                for row in f:
+                    k = row.strip().split(",")
+                    if k and k[0] == f"{w.name}_fp{prec}":
+                        roofline["traffic"] = float(k[1])
+                        roofline["traffic_source"] = k[2] if len(k) > 2 else "profiles/"
         except Exception:
             pass
 

@@ -48,16 +48,17 @@ __device__ __forceinline__ Nbr neighbours(const Geom& g, const Site& c, int r)
 }
 
 // Tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile; grid =
-// (nb0, nb1, nb2*nb3[*k]), x fastest, so CTAs are scheduled roughly in memory order.
-// `bzt` = bz + nb2*bt (blockIdx.z, or blockIdx.z with extra factors divided out).
+// (nb0[*k], nb1, nb2*nb3), dispatched x fastest, then y, then z, then t: roughly memory
+// order. (Sweeping z-slabs through all t first, to shorten the t-neighbour reuse
+// distance in L2, was measured and made no difference: profiles/r01b.md.)
 template <int LHX, int LY, int LZ, int LT>
-__device__ __forceinline__ Site tile_site(const Geom& g, uint32_t bzt)
+__device__ __forceinline__ Site tile_site(const Geom& g, uint32_t bzt, uint32_t bx = blockIdx.x)
 {
     const uint32_t bt = (g.nb[2] == 1) ? bzt : __umulhi(bzt, g.zmagic);
     const uint32_t bz = bzt - bt * (uint32_t)g.nb[2];
     const int tid = threadIdx.x;
     Site c;
-    c.hx = (int)(blockIdx.x << LHX) + (tid & ((1 << LHX) - 1));
+    c.hx = (int)(bx << LHX) + (tid & ((1 << LHX) - 1));
     c.y = (int)(blockIdx.y << LY) + ((tid >> LHX) & ((1 << LY) - 1));
     c.z = (int)(bz << LZ) + ((tid >> (LHX + LY)) & ((1 << LZ) - 1));
     c.t = (int)(bt << LT) + (tid >> (LHX + LY + LZ));
@@ -292,10 +293,12 @@ struct M<float> {
     }
     // The radius sqrt(delta(2-delta)) amplifies the absolute error of delta by 1/radius:
     // where that would exceed ~1e-6 (radius^2 < 0.12/alpha^2, probability ~1e-4) the
-    // accepted trial is recomputed with the accurate logf/cospif.
+    // accepted trial is recomputed with the accurate logf/cospif. So is
+    // every accepted trial at alpha < 2, where the error of delta itself (~4e-7/alpha,
+    // and |ln R''| times the MUFU cosine error) is no longer small against 1e-5.
     static __device__ __forceinline__ float kp_delta_refined(const Words& w, float inv_alpha, float delta)
     {
-        if (delta * (2.0f - delta) < 0.12f * inv_alpha * inv_alpha) {
+        if (delta * (2.0f - delta) < 0.12f * inv_alpha * inv_alpha || inv_alpha > 0.5f) {
             const float cs = cospif(2.0f * uniform(w.w1));
             delta = -(logf(uniform(w.w0)) + cs * cs * logf(uniform(w.w2))) * inv_alpha;
         }

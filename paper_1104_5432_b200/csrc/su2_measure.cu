@@ -55,8 +55,10 @@ __global__ void __launch_bounds__(kBlock)
     if (threadIdx.x == 0) partials[blockIdx.y * gridDim.x + blockIdx.x] = tot;
 }
 
-// Tiled form (same CTA tiles as the heat-bath kernel): grid.z carries
-// (bz, bt, parity), parity slowest. All 16 links of a site are requested before the
+// Tiled form (same CTA tiles as the heat-bath kernel): grid.x carries
+// (tile along x, parity), parity fastest, so the two CTAs that read the same 8 tiles of
+// links are scheduled back to back and the second is served by L2 (with parity slowest
+// ncu showed 2.15 GB of DRAM reads for 1.07 GB of links). All 16 links of a site are requested before the
 // first product; one partial per CTA, indexed by the linear CTA id.
 #ifndef PLAQ_MINB_F32
 #define PLAQ_MINB_F32 8
@@ -71,9 +73,8 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), sizeof(Real) == 4 ?
 {
     typedef typename LinkPtr<Real>::type L;
     __shared__ double red[kBlock / 32];
-    const uint32_t nzt = (uint32_t)(g.nb[2] * g.nb[3]);
-    const int p = blockIdx.z >= nzt ? 1 : 0;
-    const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z - (p ? nzt : 0u));
+    const int p = blockIdx.x & 1;
+    const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z, blockIdx.x >> 1);
     const int r = (c.y + c.z + c.t + p) & 1;
     const int h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
     int up[4];
@@ -231,9 +232,8 @@ static void launch_plaquette_t(const void* links, const Geom& g, const Scratch& 
                                cudaStream_t st)
 {
     typedef typename LinkPtr<Real>::type L;
-    const uint64_t nz = 2ull * (uint64_t)g.nb[2] * (uint64_t)g.nb[3];
-    if (g.tile >= 0 && nz <= 65535) {
-        const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)nz);
+    if (g.tile >= 0) {
+        const dim3 grid(2u * (unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
         *n_partials = (size_t)grid.x * grid.y * grid.z;
         if (g.tile == 0)
             plaquette_tiled_kernel<Real, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>

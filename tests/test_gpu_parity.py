@@ -42,7 +42,8 @@ def assert_links_match(gpu, ora, prec, margin=None, max_flips=0, what=""):
     return nbad
 
 
-# dims: tiled path (extents multiples of the 16x4x4x2 tile), linear path, ragged, minimal
+# dims: tiled path with the 8x4x2x2-thread tile (16,8,8,4) and the 16x4x2x1 tile (32,4,4,2),
+# linear path (8^4), ragged, minimal
 SHAPES = [(16, 8, 8, 4), (32, 4, 4, 2), (8, 8, 8, 8), (6, 4, 10, 2), (2, 2, 2, 2), (4, 2, 6, 2)]
 
 
@@ -283,3 +284,61 @@ def test_unit_norm_invariant_after_sweeps(pkg, prec):
     g = lat.get_links().astype(np.float64)
     assert np.abs((g**2).sum(-1) - 1).max() < (9e-16 if prec == 64 else 5e-7)  # 4 ulp on |a|^2
     lat.close()
+
+
+@pytest.mark.parametrize("beta", [0.3, 1.0])
+def test_fp32_small_alpha_exercises_the_accurate_refinement(pkg, beta):
+    """At small alpha = beta*k most accepted trials fall under the kernel's refinement
+    threshold (radius^2 < 0.12/alpha^2) and many trials are rejected:
+    covers the accurate logf/cospif branch and the multi-trial loop."""
+    dims, prec, mode = (16, 8, 8, 4), 32, "f32"
+    L = workloads.random_links(dims, 5, np.float32)
+    lat = pkg.Lattice(dims, prec)
+    lat.set_seed(9)
+    V = oracle.volume(dims)
+    most = 0
+    for mu, p in ((0, 0), (1, 1), (3, 0)):
+        lat.set_links(L)  # teacher-forced: a flipped accept must not feed the next sub-step
+        lat.substep(beta, 0, mu, p)
+        g = lat.get_links()
+        mg, tr = np.ones((V, 4)), np.zeros((V, 4), np.int32)
+        oracle.heatbath_substep(dims, L, beta, 9, 0, mu, p, mode, margin=mg, trials=tr)
+        most = max(most, int(tr.max()))
+        assert_links_match(g, L, prec, mg, max_flips=2, what=f"mu={mu} p={p}")
+    assert most >= 5  # the retry loop really ran
+    lat.close()
+
+
+def test_substeps_in_any_order_match_oracle(pkg):
+    """Sub-steps called out of the canonical order must not overlap their predecessor
+    (the handle only allows programmatic dependent launch after the canonical one)."""
+    dims, prec, mode = (32, 8, 8, 4), 64, "f64"
+    L = workloads.random_links(dims, 8, np.float64)
+    lat = pkg.Lattice(dims, prec)
+    lat.set_links(L)
+    lat.set_seed(3)
+    order = [(2, 1), (0, 0), (0, 1), (3, 0), (1, 1), (1, 0), (2, 0), (3, 1), (0, 0), (0, 1), (1, 0)]
+    for mu, p in order:
+        lat.substep(2.3, 1, mu, p)
+    g = lat.get_links()
+    for mu, p in order:
+        oracle.heatbath_substep(dims, L, 2.3, 3, 1, mu, p, mode)
+    assert_links_match(g, L, prec)
+    lat.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_overlapped_launches_equal_serialised_launches_bitwise(pkg, prec, monkeypatch):
+    """32^4 (many CTA waves): sweeps whose sub-steps are chained by programmatic dependent
+    launch give bit-identical links to the same sweeps with the overlap disabled."""
+    dims = (32, 32, 32, 32)
+    res = []
+    for no_pdl in ("0", "1"):
+        monkeypatch.setenv("SU2HB_NO_PDL", no_pdl)
+        lat = pkg.Lattice(dims, prec)
+        lat.init("hot", 2)
+        for i in range(3):
+            lat.sweep(6.0, i)
+        res.append(lat.get_links())
+        lat.close()
+    assert (res[0] == res[1]).all()
