@@ -4,10 +4,12 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
                     [--workload C5_64^4|C3_32^4|...] [--precision 32|64] [--headline-only]
 
-A "step" is one pass of the whole hot path over one lattice: one heat-bath sweep
-(8 checkerboard sub-steps), then the mean plaquette and the Polyakov loop of the
-new configuration (the paper's loop: "100 iterations of the heat bath method and
-the calculation of the mean average plaquette at each iteration").
+A "step" is one pass of the whole hot path over one lattice, one call of
+su2_heatbath_sweep_measure: one heat-bath sweep (8 checkerboard sub-steps), the mean
+plaquette of the new configuration (accumulated inside three of the sub-steps,
+DESIGN.md 6.5) and its Polyakov loop (the paper's loop: "100 iterations of the heat
+bath method and the calculation of the mean average plaquette at each iteration",
+PAPER.md:46).
 The random initialisation (row 1) runs once before the warm-up and is reported
 separately as `init_ms`. value = link updates/s = 4V * steps / time.
 
@@ -170,27 +172,26 @@ def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, 
     torch.cuda.synchronize()
     init_ms = e0.elapsed_time(e1)
 
-    def step(i):
-        lat.sweep(beta, i)
-        lat.measure_async(obs, i)
+    def step(i, ev_mid=None):
+        lat.sweep_measure(beta, i, obs, i, ev_mid)  # sweep + fused plaquette + Polyakov loop
 
     for i in range(warmup):
         step(i)
     lat.synchronize()
+    sweep_ev = [(ev(), ev()) for _ in range(steps)]
+    for a, b in sweep_ev:  # materialise the CUDA events (torch creates them on first record)
+        a.record()
+        b.record()
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
     n0 = lat.launch_count
-    sweep_ev = [(ev(), ev()) for _ in range(steps)]
     t_wall0 = sampler.mark() if sampler else 0.0
     start, stop = ev(), ev()
     start.record()
     for k in range(steps):
-        i = warmup + k
-        sweep_ev[k][0].record()
-        lat.sweep(beta, i)
-        sweep_ev[k][1].record()
-        lat.measure_async(obs, i)
+        sweep_ev[k][0].record()          # ... 8 sub-step kernels ...
+        step(warmup + k, sweep_ev[k][1])  # recorded by the library after the 8th sub-step
     stop.record()
     torch.cuda.synchronize()
     if dist is not None:
@@ -225,21 +226,22 @@ def time_e2e(pkg, torch, w, prec, beta, steps, warmup, seed):
     host = pinned.numpy().view(dt).reshape(w.volume, 4, 4)
     lat.init(w.start, seed)
     lat.get_links(host)
+    obs = torch.zeros(2, dtype=torch.float64, device=lat.device)
     t = []
     for k in range(warmup + steps):
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         lat.set_links(host)
-        lat.sweep(beta, k)
-        P, L = lat.measure()
+        lat.sweep_measure(beta, k, obs, 0)
         lat.get_links(host)
+        P, L = obs.cpu().numpy()
         torch.cuda.synchronize()
         t.append(time.perf_counter() - t0)
     lat.close()
     sec = float(np.mean(t[warmup:]))
     return {"value": w.links / sec, "unit": UNIT, "h2d_bytes_per_step": int(nbytes),
             "d2h_bytes_per_step": int(nbytes + 16), "ms_per_step": sec * 1e3, "steps": steps,
-            "what": "su2_set_links(pinned host) + su2_heatbath_sweep + su2_measure + su2_get_links(pinned host)"}
+            "what": "su2_set_links(pinned host) + su2_heatbath_sweep_measure + su2_get_links(pinned host) + 16 B of observables"}
 
 
 # ------------------------------------------------------------------------------- oracle
@@ -321,6 +323,8 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_1104_5432_b200 import build as lib_build
+    lib_build.build()  # no-op unless a source is newer than the in-tree library
     pkg.lib()
     peak, peak_src = measured_peaks()
     w = workloads.BY_NAME[args.workload]
@@ -369,7 +373,7 @@ def main():
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
         "config": {"workload": f"{w.name} beta={args.beta} start={w.start} seed={args.seed}",
-                   "precision": prec, "step": "1 heat-bath sweep (8 sub-steps) + mean plaquette + Polyakov loop",
+                   "precision": prec, "step": "su2_heatbath_sweep_measure: 1 heat-bath sweep (8 sub-steps, plaquette fused into 3 of them) + Polyakov loop",
                    "l2": (("inputs larger than L2 (%d MiB lattice vs 126 MiB L2), no flush needed"
                            if (w.links * 4 * prec // 8 >> 20) > 126 else
                            "lattice %d MiB is L2-resident by nature of the workload; no flush between steps")

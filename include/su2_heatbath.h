@@ -121,6 +121,20 @@ SU2_API int su2_measure(su2_lattice* lat, double* plaquette_out, double* polyako
  * ([device], caller-owned). No synchronisation. */
 SU2_API int su2_measure_async(su2_lattice* lat, double* dev_out, size_t index);
 
+/* The paper's loop body in one call ("100 iterations of the heat bath method and
+ * the calculation of the mean average plaquette at each iteration"): one sweep exactly as
+ * su2_heatbath_sweep, then the mean plaquette [R10] and the Polyakov loop [R11] of the NEW
+ * configuration at dev_out[2*index], dev_out[2*index+1] ([device], caller-owned doubles).
+ * The plaquette is accumulated inside the sub-steps (mu >= 1, parity 1) as 1/2 Tr(U' w), w =
+ * the staple terms of the directions nu < mu, which sums every plaquette of the final
+ * configuration once; it equals su2_mean_plaquette after the sweep to rounding
+ * (fp64 accumulation, fixed order) and saves that kernel's pass over the lattice.
+ * event_after_sweep: NULL, or a cudaEvent_t the library records on the handle's stream
+ * between the 8th sub-step and the two reduction kernels (bench.py times the sub-steps with it).
+ * Asynchronous, no synchronisation. Errors as su2_heatbath_sweep, plus SU2_EARG for NULL dev_out. */
+SU2_API int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_t sweep_idx, double* dev_out,
+                                       size_t index, void* event_after_sweep);
+
 /* NEXT-1 (eq. 3): on-axis Polyakov-loop correlator
  * C(r) = < l(x) l(x + r e_i) >, averaged over all spatial x and the 3 spatial axes i,
  * r = 1..rmax (rmax <= min spatial extent / 2), l(x) = 1/2 Tr L(x) (real in SU(2)).

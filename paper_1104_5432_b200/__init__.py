@@ -33,6 +33,8 @@ _SIGNATURES = {
     "su2_set_seed": (C.c_int, [C.c_void_p, C.c_uint64]),
     "su2_heatbath_sweep": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32]),
     "su2_heatbath_substep": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32, C.c_int, C.c_int]),
+    "su2_heatbath_sweep_measure": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32, C.c_void_p, C.c_size_t,
+                                             C.c_void_p]),
     "su2_mean_plaquette": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "su2_polyakov_loop": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "su2_measure": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
@@ -121,6 +123,11 @@ def su2_heatbath_sweep(h, beta, sweep_idx):
 
 def su2_heatbath_substep(h, beta, sweep_idx, mu, parity):
     _check(lib().su2_heatbath_substep(h, beta, sweep_idx, mu, parity), h)
+
+
+def su2_heatbath_sweep_measure(h, beta, sweep_idx, dev_out_ptr, index, event_after_sweep=0):
+    _check(lib().su2_heatbath_sweep_measure(h, beta, sweep_idx, C.c_void_p(dev_out_ptr), index,
+                                            C.c_void_p(event_after_sweep)), h)
 
 
 def su2_mean_plaquette(h):
@@ -215,6 +222,11 @@ class Lattice:
 
     def sweep(self, beta, sweep_idx):
         su2_heatbath_sweep(self.h, beta, sweep_idx)
+
+    def sweep_measure(self, beta, sweep_idx, dev_out, index, event_after_sweep=None):
+        """dev_out: torch float64 device tensor; event_after_sweep: a recorded-once torch.cuda.Event."""
+        ev = event_after_sweep.cuda_event if event_after_sweep is not None else 0
+        su2_heatbath_sweep_measure(self.h, beta, sweep_idx, dev_out.data_ptr(), index, ev)
 
     def substep(self, beta, sweep_idx, mu, parity):
         su2_heatbath_substep(self.h, beta, sweep_idx, mu, parity)

@@ -55,12 +55,13 @@ static int fail(su2_lattice* lat, int code, const char* what, cudaError_t ce = c
 
 // launch sub-step (mu, parity); it may overlap the tail of the previous launch only if
 // that was its canonical predecessor [R4] on this handle
-static void enqueue_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, int mu, int parity)
+static void enqueue_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, int mu, int parity,
+                            double* epart = nullptr)
 {
     const int idx = 2 * mu + parity;
     const bool overlap = lat->pdl && lat->last_substep == (idx + 7) % 8;
     lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, parity, beta, lat->seed,
-                                             sweep_idx, lat->sc.err, overlap, lat->stream);
+                                             sweep_idx, lat->sc.err, epart, overlap, lat->stream);
     lat->last_substep = idx;
 }
 
@@ -121,6 +122,7 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
     const uint64_t v3 = (uint64_t)Nx * Ny * Nz;
     lat->sc.n_partials = partials_needed(g);
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.partials, lat->sc.n_partials * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.epart, 3 * heatbath_ctas(g) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.field, v3 * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.out, (2 + kMaxR) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.err, sizeof(int));
@@ -151,6 +153,7 @@ extern "C" int su2_lattice_destroy(su2_lattice* lat)
     if (!lat) return SU2_OK;
     if (lat->owns_links && lat->links) cudaFree(lat->links);
     if (lat->sc.partials) cudaFree(lat->sc.partials);
+    if (lat->sc.epart) cudaFree(lat->sc.epart);
     if (lat->sc.field) cudaFree(lat->sc.field);
     if (lat->sc.out) cudaFree(lat->sc.out);
     if (lat->sc.err) cudaFree(lat->sc.err);
@@ -209,6 +212,27 @@ extern "C" int su2_heatbath_sweep(su2_lattice* lat, double beta, uint32_t sweep_
     for (int mu = 0; mu < 4; ++mu)      // [R4] direction outer,
         for (int p = 0; p < 2; ++p)     //      parity inner
             enqueue_substep(lat, beta, sweep_idx, mu, p);
+    CK(lat, cudaGetLastError());
+    return SU2_OK;
+}
+
+extern "C" int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_t sweep_idx, double* dev_out,
+                                          size_t index, void* event_after_sweep)
+{
+    ENTER(lat);
+    if (int rc = check_beta(lat, beta)) return rc;
+    if (!dev_out) return fail(lat, SU2_EARG, "su2_heatbath_sweep_measure: NULL dev_out");
+    const size_t ctas = heatbath_ctas(lat->g);
+    for (int mu = 0; mu < 4; ++mu)
+        for (int p = 0; p < 2; ++p)
+            enqueue_substep(lat, beta, sweep_idx, mu, p, (p == 1 && mu >= 1) ? lat->sc.epart + (mu - 1) * ctas : nullptr);
+    NOT_A_SUBSTEP(lat);
+    if (event_after_sweep) CK(lat, cudaEventRecord((cudaEvent_t)event_after_sweep, lat->stream));
+    // the three partial sets cover every plaquette of the new configuration once
+    lat->launches += launch_final_sum(lat->sc.epart, 3 * ctas, 1.0 / (6.0 * 2.0 * (double)lat->g.vh),
+                                      dev_out + 2 * index, lat->stream);
+    lat->launches +=
+        launch_polyakov(lat->links, lat->g, lat->precision, lat->sc, dev_out + 2 * index + 1, lat->stream);
     CK(lat, cudaGetLastError());
     return SU2_OK;
 }

@@ -342,6 +342,7 @@ struct __align__(16) HbParams {
     const typename LinkPtr<Real>::type* same[4];  // U_nu on the parity being updated
     const typename LinkPtr<Real>::type* oppo[4];  // U_nu on the other parity
     typename LinkPtr<Real>::type* out;            // U_mu on the parity being updated
+    double* epart;                                // fused plaquette: one partial per CTA (MEAS kernels)
     Real inv_beta;
     uint32_t sweep;
 };

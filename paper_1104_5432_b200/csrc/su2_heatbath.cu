@@ -25,8 +25,15 @@ namespace su2 {
 // dependent round trip, or spills) than they hide. The predecessor's output is read
 // through L2 (ld.global.cg): its lines may not be taken from an L1 that an overlapping
 // launch did not invalidate. Launched without the attribute the wait is a no-op.
-template <typename Real, int MU, int P>
-__device__ __forceinline__ void heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
+//
+// Fused plaquette. MEAS is used only for P = 1, MU >= 1: the return value
+// is 1/2 Tr(U' w), w = the staple terms of the directions nu < MU, i.e. the sum of the
+// plaquettes of the planes (nu, MU), nu < MU, through the new link. Those planes are not
+// touched by any later sub-step of the sweep and each of their plaquettes holds exactly
+// one odd-parity mu-link, so the three kernels (1,1), (2,1), (3,1) together sum every
+// plaquette of the final configuration exactly once.
+template <typename Real, int MU, int P, bool MEAS>
+__device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
                                               int* __restrict__ err)
 {
     typedef typename LinkPtr<Real>::type L;
@@ -64,11 +71,12 @@ __device__ __forceinline__ void heatbath_site(const Geom& g, const Site& c, cons
 
     // [R3] staple sum, nu ascending, forward then backward, products left to right;
     // the second product of every term accumulates straight into v (FMA chains).
-    Quat<Real> v = {0, 0, 0, 0};
+    Quat<Real> v = {0, 0, 0, 0}, w = {0, 0, 0, 0};
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         qmac<false, true>(v, qmul<false, true>(a[i], b[i]), cc[i]);    // (a b^+) c^+
         qmac<false, false>(v, qmul<true, true>(a2[i], b2[i]), c2[i]);  // (a2^+ b2^+) c2
+        if (MEAS && i == MU - 1) w = v;  // nu = 0..MU-1 are the first MU terms
     }
 
     const Real k2 = v.a0 * v.a0 + v.a1 * v.a1 + v.a2 * v.a2 + v.a3 * v.a3;
@@ -109,6 +117,7 @@ __device__ __forceinline__ void heatbath_site(const Geom& g, const Site& c, cons
     const Real inv = M<Real>::rsqrt(u.a0 * u.a0 + u.a1 * u.a1 + u.a2 * u.a2 + u.a3 * u.a3);
     u.a0 *= inv; u.a1 *= inv; u.a2 *= inv; u.a3 *= inv;
     stq(hp.out + (uint32_t)h, u);
+    return MEAS ? u.a0 * w.a0 - u.a1 * w.a1 - u.a2 * w.a2 - u.a3 * w.a3 : (Real)0;  // 1/2 Tr(U' w)
 }
 
 // Resident CTAs per SM that ptxas must allow: this is the register budget that lets it
@@ -130,29 +139,41 @@ struct MinBlocks<double> {
 
 // tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile;
 // grid = (nb0, nb1, nb2*nb3): x fastest, so CTAs are scheduled roughly in memory order.
-template <typename Real, int MU, int P, int LHX, int LY, int LZ, int LT>
+template <typename Real, int MU, int P, bool MEAS, int LHX, int LY, int LZ, int LT>
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::value)
     heatbath_tiled_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
     const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z);
-    heatbath_site<Real, MU, P>(g, c, hp, err);
+    const Real e = heatbath_site<Real, MU, P, MEAS>(g, c, hp, err);
+    if (MEAS) {  // one fp64 partial per CTA, fixed order
+        __shared__ double red[kBlock / 32];
+        const double tot = block_sum((double)e, red);
+        if (threadIdx.x == 0) hp.epart[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = tot;
+    }
 }
 
 // linear launch: thread i <-> half-index h = i; any even extents
-template <typename Real, int MU, int P>
+template <typename Real, int MU, int P, bool MEAS>
 __global__ void __launch_bounds__(kBlock)
     heatbath_linear_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
     const uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
-    if (h >= g.vh) return;
-    Site c;
-    uint32_t q = h / (uint32_t)g.nxh;
-    c.hx = (int)(h - q * (uint32_t)g.nxh);
-    uint32_t q2 = q / (uint32_t)g.n[1];
-    c.y = (int)(q - q2 * (uint32_t)g.n[1]);
-    c.t = (int)(q2 / (uint32_t)g.n[2]);
-    c.z = (int)(q2 - (uint32_t)c.t * (uint32_t)g.n[2]);
-    heatbath_site<Real, MU, P>(g, c, hp, err);
+    Real e = 0;
+    if (h < g.vh) {
+        Site c;
+        uint32_t q = h / (uint32_t)g.nxh;
+        c.hx = (int)(h - q * (uint32_t)g.nxh);
+        uint32_t q2 = q / (uint32_t)g.n[1];
+        c.y = (int)(q - q2 * (uint32_t)g.n[1]);
+        c.t = (int)(q2 / (uint32_t)g.n[2]);
+        c.z = (int)(q2 - (uint32_t)c.t * (uint32_t)g.n[2]);
+        e = heatbath_site<Real, MU, P, MEAS>(g, c, hp, err);
+    }
+    if (MEAS) {
+        __shared__ double red[kBlock / 32];
+        const double tot = block_sum((double)e, red);
+        if (threadIdx.x == 0) hp.epart[blockIdx.x] = tot;
+    }
 }
 
 // [R9] init: one thread per link of the device layout
@@ -221,9 +242,9 @@ static void launch_ex(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStrea
     cudaLaunchKernelEx(&cfg, kernel, args...);
 }
 
-template <typename Real, int MU, int P>
+template <typename Real, int MU, int P, bool MEAS>
 static int launch_substep_t(void* links, const Geom& g, double beta, uint64_t seed, uint32_t sweep, int* err,
-                            bool overlap, cudaStream_t st)
+                            double* epart, bool overlap, cudaStream_t st)
 {
     typedef typename LinkPtr<Real>::type L;
     HbParams<Real> hp;
@@ -235,43 +256,63 @@ static int launch_substep_t(void* links, const Geom& g, double beta, uint64_t se
         hp.oppo[nu] = (const L*)links + (size_t)((1 - P) * 4 + nu) * g.vh;
     }
     hp.out = (L*)links + (size_t)(P * 4 + MU) * g.vh;
+    hp.epart = epart;
     const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
     if (g.tile == 0) {
-        launch_ex(heatbath_tiled_kernel<Real, MU, P, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>, grid,
-                  dim3(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3])), st, overlap, g, hp, err);
+        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>,
+                  grid, dim3(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3])), st, overlap, g, hp,
+                  err);
     } else if (g.tile == 1) {
-        launch_ex(heatbath_tiled_kernel<Real, MU, P, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3]>, grid,
-                  dim3(1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3])), st, overlap, g, hp, err);
+        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3]>,
+                  grid, dim3(1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3])), st, overlap, g, hp,
+                  err);
     } else {
-        const unsigned nblk = (g.vh + kBlock - 1) / kBlock;
-        launch_ex(heatbath_linear_kernel<Real, MU, P>, dim3(nblk), dim3(kBlock), st, overlap, g, hp, err);
+        launch_ex(heatbath_linear_kernel<Real, MU, P, MEAS>, dim3((unsigned)heatbath_ctas(g)), dim3(kBlock), st,
+                  overlap, g, hp, err);
     }
     return 1;
 }
 
+// number of CTAs (= fused-plaquette partials) of one heat-bath launch
+size_t heatbath_ctas(const Geom& g)
+{
+    if (g.tile >= 0) return (size_t)g.nb[0] * g.nb[1] * g.nb[2] * g.nb[3];
+    return ((size_t)g.vh + kBlock - 1) / kBlock;
+}
+
 template <typename Real>
 static int launch_substep_p(void* links, const Geom& g, int mu, int parity, double beta, uint64_t seed,
-                            uint32_t sweep, int* err, bool overlap, cudaStream_t st)
+                            uint32_t sweep, int* err, double* epart, bool overlap, cudaStream_t st)
 {
+    if (epart && parity == 1 && mu >= 1) {  // the three measuring kernels
+        switch (mu) {
+            case 1: return launch_substep_t<Real, 1, 1, true>(links, g, beta, seed, sweep, err, epart, overlap, st);
+            case 2: return launch_substep_t<Real, 2, 1, true>(links, g, beta, seed, sweep, err, epart, overlap, st);
+            default: return launch_substep_t<Real, 3, 1, true>(links, g, beta, seed, sweep, err, epart, overlap, st);
+        }
+    }
     switch (mu * 2 + parity) {
-        case 0: return launch_substep_t<Real, 0, 0>(links, g, beta, seed, sweep, err, overlap, st);
-        case 1: return launch_substep_t<Real, 0, 1>(links, g, beta, seed, sweep, err, overlap, st);
-        case 2: return launch_substep_t<Real, 1, 0>(links, g, beta, seed, sweep, err, overlap, st);
-        case 3: return launch_substep_t<Real, 1, 1>(links, g, beta, seed, sweep, err, overlap, st);
-        case 4: return launch_substep_t<Real, 2, 0>(links, g, beta, seed, sweep, err, overlap, st);
-        case 5: return launch_substep_t<Real, 2, 1>(links, g, beta, seed, sweep, err, overlap, st);
-        case 6: return launch_substep_t<Real, 3, 0>(links, g, beta, seed, sweep, err, overlap, st);
-        default: return launch_substep_t<Real, 3, 1>(links, g, beta, seed, sweep, err, overlap, st);
+        case 0: return launch_substep_t<Real, 0, 0, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
+        case 1: return launch_substep_t<Real, 0, 1, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
+        case 2: return launch_substep_t<Real, 1, 0, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
+        case 3: return launch_substep_t<Real, 1, 1, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
+        case 4: return launch_substep_t<Real, 2, 0, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
+        case 5: return launch_substep_t<Real, 2, 1, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
+        case 6: return launch_substep_t<Real, 3, 0, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
+        default: return launch_substep_t<Real, 3, 1, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
     }
 }
 
 // `overlap` may be true only if the launch before this one on `st` was the canonical
-// predecessor sub-step [R4] of the same lattice (see heatbath_site).
+// predecessor sub-step [R4] of the same lattice (see heatbath_site). `epart` (nullable):
+// where the sub-steps (mu >= 1, parity 1) store their heatbath_ctas(g) fused-plaquette
+// partials; ignored by the other sub-steps.
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
-                            uint64_t seed, uint32_t sweep, int* err, bool overlap, cudaStream_t st)
+                            uint64_t seed, uint32_t sweep, int* err, double* epart, bool overlap, cudaStream_t st)
 {
-    return precision == 32 ? launch_substep_p<float>(links, g, mu, parity, beta, seed, sweep, err, overlap, st)
-                           : launch_substep_p<double>(links, g, mu, parity, beta, seed, sweep, err, overlap, st);
+    return precision == 32
+               ? launch_substep_p<float>(links, g, mu, parity, beta, seed, sweep, err, epart, overlap, st)
+               : launch_substep_p<double>(links, g, mu, parity, beta, seed, sweep, err, epart, overlap, st);
 }
 
 int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st)

@@ -26,6 +26,7 @@ constexpr int kBlock = 256;                 // block size of every other kernel;
 struct Scratch {
     double* partials;   // [device] block partial sums (plaquette | polyakov | correlator)
     size_t n_partials;  // capacity in doubles
+    double* epart;      // [device] fused plaquette partials: 3 * heatbath_ctas(g) doubles
     double* field;      // [device] l(x) of the Polyakov kernel, V/Nt doubles
     double* out;        // [device] 2 + kMaxR doubles: plaquette, polyakov, correlator
     int* err;           // [device] sticky error flags (bit 0: KP trial cap hit)
@@ -39,7 +40,9 @@ size_t partials_needed(const Geom& g);
 // each returns the number of kernels it enqueued (0 on launch failure; check cudaGetLastError)
 int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st);
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
-                            uint64_t seed, uint32_t sweep, int* err, bool overlap, cudaStream_t st);
+                            uint64_t seed, uint32_t sweep, int* err, double* epart, bool overlap, cudaStream_t st);
+size_t heatbath_ctas(const Geom& g);
+int launch_final_sum(const double* partials, size_t n, double scale, double* dev_dst, cudaStream_t st);
 int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
                      cudaStream_t st);
 int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,

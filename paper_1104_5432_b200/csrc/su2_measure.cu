@@ -263,6 +263,12 @@ int launch_plaquette(const void* links, const Geom& g, int precision, const Scra
     return 2;
 }
 
+int launch_final_sum(const double* partials, size_t n, double scale, double* dev_dst, cudaStream_t st)
+{
+    final_sum_kernel<<<1, 1024, 0, st>>>(partials, n, scale, dev_dst);
+    return 1;
+}
+
 int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
                     cudaStream_t st)
 {

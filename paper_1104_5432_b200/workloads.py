@@ -68,3 +68,29 @@ def smooth_links(dims, seed: int, eps: float, dtype=np.float64) -> np.ndarray:
     a[..., 1:] = eps * rng.standard_normal((V, D, 3))
     a /= np.linalg.norm(a, axis=-1, keepdims=True)
     return np.ascontiguousarray(a.astype(dtype))
+
+
+def degenerate_staple_links(dims, s: int, mu: int, dtype=np.float64) -> np.ndarray:
+    """Cold lattice in which the staple sum of link (site s, direction mu) vanishes
+    exactly: U_mu(x - nu) = -1 for the three nu != mu turns every backward term into
+    -1 against the +1 of the forward terms (the [R8] measure-zero case, built by hand).
+    Needs every extent >= 4 so that the flipped links are distinct from the others."""
+    D = len(dims)
+    V = int(np.prod(dims))
+    a = np.zeros((V, D, 4), dtype=dtype)
+    a[..., 0] = 1.0
+    x = []
+    r = s
+    for n in dims:
+        x.append(r % n)
+        r //= n
+    for nu in range(D):
+        if nu == mu:
+            continue
+        y = list(x)
+        y[nu] = (y[nu] - 1) % dims[nu]
+        sy = 0
+        for d in reversed(range(D)):
+            sy = sy * dims[d] + y[d]
+        a[sy, mu, 0] = -1.0
+    return a

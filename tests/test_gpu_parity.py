@@ -25,6 +25,8 @@ def pkg():
     import torch
     assert torch.cuda.is_available(), "-m gpu tests need a CUDA device"
     import paper_1104_5432_b200 as p
+    from paper_1104_5432_b200 import build
+    build.build()  # no-op unless a source is newer than the library
     p.lib()
     return p
 
@@ -342,3 +344,50 @@ def test_overlapped_launches_equal_serialised_launches_bitwise(pkg, prec, monkey
         res.append(lat.get_links())
         lat.close()
     assert (res[0] == res[1]).all()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_degenerate_staple_matches_oracle(pkg, prec):
+    """[R8] on the hand-built k = 0 lattice: the kernel takes the same Haar branch."""
+    dims, mu = (4, 4, 4, 4), 1
+    mode = MODE[prec]
+    for s in (37, 38):  # one site of each parity
+        L = workloads.degenerate_staple_links(dims, s, mu, oracle.dtype(mode))
+        par = sum((s // int(np.prod(dims[:d]))) % dims[d] for d in range(4)) % 2
+        lat = pkg.Lattice(dims, prec)
+        lat.set_links(L)
+        lat.set_seed(5)
+        lat.substep(2.3, 0, mu, par)
+        g = lat.get_links()
+        tr = np.full((oracle.volume(dims), 4), -1, np.int32)
+        oracle.heatbath_substep(dims, L, 2.3, 5, 0, mu, par, mode, trials=tr)
+        assert tr[s, mu] == 0  # the oracle took the degenerate branch there
+        assert np.abs(g[s, mu].astype(np.float64) - L[s, mu].astype(np.float64)).max() < (2e-15 if prec == 64 else 1e-6)
+        assert_links_match(g, L, prec)
+        lat.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", SHAPES + [(12, 6, 4, 6)])
+def test_sweep_measure_fused_plaquette_matches_oracle_and_standalone_kernel(pkg, dims, prec):
+    """su2_heatbath_sweep_measure: same links as su2_heatbath_sweep (bitwise); its fused
+    plaquette and its Polyakov loop equal the oracle's on the new configuration."""
+    import torch
+    mode = MODE[prec]
+    L = workloads.random_links(dims, 13, oracle.dtype(mode))
+    obs = torch.zeros(6, dtype=torch.float64, device="cuda")
+    a, b = pkg.Lattice(dims, prec), pkg.Lattice(dims, prec)
+    for lat in (a, b):
+        lat.set_links(L)
+        lat.set_seed(4)
+    for i in range(3):
+        a.sweep(2.3, i)
+        b.sweep_measure(2.3, i, obs, i)
+        ga, gb = a.get_links(), b.get_links()
+        assert (ga == gb).all()
+        P, Lp = obs.cpu().numpy()[2 * i: 2 * i + 2]
+        assert abs(P - oracle.mean_plaquette(dims, gb, mode)) < PTOL[prec]
+        assert abs(Lp - oracle.polyakov_loop(dims, gb, mode)) < 10 * PTOL[prec]
+        assert abs(P - a.mean_plaquette()) < (1e-13 if prec == 64 else 2e-7)
+    a.close()
+    b.close()

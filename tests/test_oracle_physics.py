@@ -318,3 +318,21 @@ def test_fp32_modes_track_fp64_on_one_teacher_forced_sweep():
     # spread; with 1024 links the expected number of flips is ~1e-4: demand none.
     assert not bad.any()
     assert abs(oracle.mean_plaquette(dims, A, "f32") - oracle.mean_plaquette(dims, B, "f32x")) < 1e-6
+
+
+def test_degenerate_staple_gives_haar_element_independent_of_beta():
+    """[R8]: k = 0 exactly on a hand-built lattice -> the new link is the Haar element of the
+    n = 0 words: unit norm, no KP trial, the same for every beta, different per sweep_idx."""
+    from paper_1104_5432_b200 import workloads
+    dims, s, mu = [4, 4, 4, 4], 37, 1
+    L = workloads.degenerate_staple_links(dims, s, mu)
+    assert np.abs(oracle.staple(dims, L, s, mu)).max() == 0.0
+    u1, tr1, _ = oracle.heatbath_link(dims, L, 2.3, 5, 0, s, mu)
+    u2, tr2, _ = oracle.heatbath_link(dims, L, 6.0, 5, 0, s, mu)
+    u3, _, _ = oracle.heatbath_link(dims, L, 6.0, 5, 1, s, mu)
+    assert tr1 == 0 and tr2 == 0
+    assert (u1 == u2).all() and not (u1 == u3).all()
+    assert abs(np.linalg.norm(u1) - 1) < 1e-15
+    # a neighbouring link with a non-zero staple is updated normally
+    u4, tr4, _ = oracle.heatbath_link(dims, L, 2.3, 5, 0, s + 1, mu)
+    assert tr4 >= 1
