@@ -27,9 +27,15 @@ def test_sampled_link_parity_at_bench_sizes(dims, prec, start, beta):
     seed = 1
     lat = pkg.Lattice(dims, prec)
     lat.init(start, seed)
-    lat.sweep(beta, 0)
-    lat.sweep(beta, 1)  # a cold start needs a sweep to become non-trivial
+    import torch
+    obs = torch.zeros(4, dtype=torch.float64, device="cuda")
+    lat.sweep_measure(beta, 0, obs, 0)  # the call bench.py times
+    lat.sweep_measure(beta, 1, obs, 1)  # a cold start needs a sweep to become non-trivial
     before = lat.get_links()
+    # fused plaquette / Polyakov loop of the call against the standalone kernels at full size
+    P_fused, L_fused = obs.cpu().numpy()[2:4]
+    assert abs(P_fused - lat.mean_plaquette()) < (1e-13 if prec == 64 else 2e-7)
+    assert abs(L_fused - lat.polyakov_loop()) < 1e-15
     V = oracle.volume(dims)
     rng = np.random.default_rng(5)
     n_sample = 600
