@@ -245,19 +245,47 @@ def time_e2e(pkg, torch, w, prec, beta, steps, warmup, seed):
 
 
 # ------------------------------------------------------------------------------- oracle
-def oracle_sample(w, prec, beta, seed, n_substeps=2):
-    """The oracle as it stands on one host core: the first `n_substeps` sub-steps
-    (mu=0; parity 0,1) of sweep 0 on the workload's own lattice."""
-    import oracle
-    mode = "f32" if prec == 32 else "f64"
-    links = oracle.init(w.dims, w.start, seed, mode)
-    t0 = time.perf_counter()
-    done = 0
-    for j in range(n_substeps):
-        oracle.heatbath_substep(w.dims, links, beta, seed, 0, j // 2, j % 2, mode)
-        done += w.volume // 2
-    sec = time.perf_counter() - t0
-    return done / sec, sec, done
+class OracleSlab:
+    """The oracle as it stands (gcc -O2, serial, one host core) on a BOUNDED sample of the
+    workload: the same lattice cut down to its first Nt' time slices (periodic), Nt' even,
+    chosen so that one step costs about `seconds_per_step`. A step is the whole hot path:
+    one heat-bath sweep + mean plaquette + Polyakov loop, continuing one chain."""
+
+    def __init__(self, w, prec, beta, seed, seconds_per_step):
+        import oracle
+        self.oracle, self.w, self.beta, self.seed = oracle, w, beta, seed
+        self.mode = "f32" if prec == 32 else "f64"
+        nx, ny, nz, nt = w.dims
+        # calibrate on the 2-slice slab
+        self.dims = (nx, ny, nz, 2)
+        self.links = oracle.init(self.dims, w.start, seed, self.mode)
+        rate = self._step(0)[0]  # link updates/s
+        want = seconds_per_step * rate / (4.0 * nx * ny * nz)
+        nts = int(min(nt, max(2, 2 * round(want / 2.0))))
+        if nts != 2:
+            self.dims = (nx, ny, nz, nts)
+            self.links = oracle.init(self.dims, w.start, seed, self.mode)
+        self.k = 1
+
+    def _step(self, k):
+        o = self.oracle
+        t0 = time.perf_counter()
+        o.heatbath_sweep(self.dims, self.links, self.beta, self.seed, k, self.mode)
+        P = o.mean_plaquette(self.dims, self.links, self.mode)
+        L = o.polyakov_loop(self.dims, self.links, self.mode)
+        sec = time.perf_counter() - t0
+        n = 4 * int(np.prod(self.dims))
+        return n / sec, sec, n, P, L
+
+    def step(self):
+        r = self._step(self.k)
+        self.k += 1
+        return r
+
+    def describe(self, prec):
+        return (f"1 oracle step (heat-bath sweep + mean plaquette + Polyakov loop) on the first {self.dims[3]} of "
+                f"{self.w.dims[3]} time slices of the {self.w.name} lattice = {4 * int(np.prod(self.dims))} link "
+                f"updates per step, fp{prec} oracle mode, gcc -O2, serial")
 
 
 def run_reference(args):
@@ -267,25 +295,24 @@ def run_reference(args):
     from paper_1104_5432_b200 import workloads
     w = workloads.BY_NAME[args.workload]
     prec = args.precision
-    # bounded sample per step: one sub-step pair on 32^4-sized work (the 64^4 lattice itself for C5)
-    vals, secs, n = [], [], 0
+    # the whole --steps K --warmup W run is sized to about two minutes of host time
+    slab = OracleSlab(w, prec, args.beta, args.seed, args.ref_seconds / max(1, args.warmup + args.steps))
+    vals, secs = [], []
     for k in range(args.warmup + args.steps):
-        v, s, n = oracle_sample(w, prec, args.beta, args.seed, n_substeps=args.ref_substeps)
+        v, sec, n, P, L = slab.step()
         if k >= args.warmup:
             vals.append(v)
-            secs.append(s)
-    value = float(np.mean(vals))
-    sample = (f"{args.ref_substeps} heat-bath sub-step(s) (mu=0) of sweep 0 on the {w.name} lattice "
-              f"({n} link updates per step), fp{prec} oracle mode, gcc -O2, serial")
+            secs.append(sec)
+    value = float(np.sum([4 * np.prod(slab.dims)] * len(secs)) / np.sum(secs))
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(secs)) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
         "config": {"workload": f"{w.name} beta={args.beta} start={w.start} (bounded sample)", "precision": prec},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": slab.describe(prec)},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-        "gpu_launches": 0,
+        "gpu_launches": 0, "plaquette_last": P, "polyakov_last": L,
     }
     print(json.dumps(line))
     return 0
@@ -304,7 +331,8 @@ def main():
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--headline-only", action="store_true", help="skip the other metric points, e2e and cpu_baseline")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--ref-substeps", type=int, default=2)
+    ap.add_argument("--ref-seconds", type=float, default=120.0, help="host time the whole reference run may take")
+    ap.add_argument("--cpu-baseline-seconds", type=float, default=12.0)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -405,11 +433,10 @@ def main():
             }
         line["workloads"] = others
         line["e2e"] = time_e2e(pkg, torch, w, prec, args.beta, args.e2e_steps, 1, args.seed)
-        v, sec, n = oracle_sample(w, prec, args.beta, args.seed, n_substeps=args.ref_substeps)
+        slab = OracleSlab(w, prec, args.beta, args.seed, args.cpu_baseline_seconds)
+        v, sec, n, _, _ = slab.step()
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                "sample": f"{args.ref_substeps} heat-bath sub-steps (mu=0, both parities) of sweep 0 on "
-                                          f"the {w.name} lattice = {n} link updates in {sec:.1f} s, fp{prec} oracle "
-                                          f"mode, gcc -O2, serial"}
+                                "sample": slab.describe(prec) + f" ({sec:.1f} s)"}
     sampler.stop()
     if world > 1:
         dist.barrier()
