@@ -38,6 +38,7 @@ import numpy as np
 
 METRIC = "su2_heatbath_link_updates_per_s"
 UNIT = "link updates/s"
+COOL_DOWN_S = 2.0  # idle time before each workload (outside every timed region)
 BYTES_PER_UPDATE = {32: 128, 64: 256}  # 8 quaternions per link update
 
 
@@ -160,6 +161,7 @@ def dist_env():
 # ------------------------------------------------------------------------------- ours
 def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, dist=None):
     """Device-resident timing of `steps` steps. Returns a dict of measurements."""
+    time.sleep(COOL_DOWN_S)  # every workload starts from the same power state, whatever ran before it
     lat = pkg.Lattice(w.dims, prec)
     ev = lambda: torch.cuda.Event(enable_timing=True)
     obs = torch.zeros(2 * (steps + warmup), dtype=torch.float64, device=lat.device)
@@ -172,11 +174,12 @@ def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, 
     torch.cuda.synchronize()
     init_ms = e0.elapsed_time(e1)
 
-    def step(i, ev_mid=None):
-        lat.sweep_measure(beta, i, obs, i, ev_mid)  # sweep + fused plaquette + Polyakov loop
-
+    # warm-up, then the timed region: EXACTLY `steps` steps, one su2_heatbath_sweep_measure call
+    # each, with a CUDA-event pair around the 8 sub-step kernels of every step (the second
+    # event of a pair is recorded by the library between the 8th sub-step and the reductions):
+    # the heat-bath kernel's average launch duration for the roofline comes from the SAME region
     for i in range(warmup):
-        step(i)
+        lat.sweep_measure(beta, i, obs, i)
     lat.synchronize()
     sweep_ev = [(ev(), ev()) for _ in range(steps)]
     for a, b in sweep_ev:  # materialise the CUDA events (torch creates them on first record)
@@ -190,8 +193,8 @@ def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, 
     start, stop = ev(), ev()
     start.record()
     for k in range(steps):
-        sweep_ev[k][0].record()          # ... 8 sub-step kernels ...
-        step(warmup + k, sweep_ev[k][1])  # recorded by the library after the 8th sub-step
+        sweep_ev[k][0].record()
+        lat.sweep_measure(beta, warmup + k, obs, warmup + k, sweep_ev[k][1])
     stop.record()
     torch.cuda.synchronize()
     if dist is not None:
@@ -201,9 +204,20 @@ def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, 
     launches = lat.launch_count - n0
     ms = start.elapsed_time(stop)
     sweep_ms = float(np.mean([a.elapsed_time(b) for a, b in sweep_ev]))
-    o = obs.cpu().numpy().reshape(-1, 2)
+    o = obs.cpu().numpy().reshape(-1, 2).copy()
+
+    # extra (not the headline): the same `steps` steps as ONE su2_run call — the step captured as
+    # a CUDA graph and replayed, no host work per step (matters on small lattices)
+    s2, e2 = ev(), ev()
+    s2.record()
+    lat.run(beta, warmup + steps, steps, obs)
+    e2.record()
+    torch.cuda.synchronize()
+    lat.synchronize()
+    ms_run = s2.elapsed_time(e2) / steps
     res = {
         "ms_total": ms, "ms_per_step": ms / steps, "sweep_ms": sweep_ms, "init_ms": init_ms,
+        "ms_per_step_run": ms_run,
         "launches": int(launches), "plaquette_last": float(o[warmup + steps - 1, 0]),
         "polyakov_last": float(o[warmup + steps - 1, 1]), "t_wall": (t_wall0, t_wall1),
         "links": w.links,
@@ -406,10 +420,14 @@ def main():
                            if (w.links * 4 * prec // 8 >> 20) > 126 else
                            "lattice %d MiB is L2-resident by nature of the workload; no flush between steps")
                           % (w.links * 4 * prec // 8 >> 20)),
+                   "cool_down": f"{COOL_DOWN_S} s idle before each workload's warm-up (power state independent of the workload before)",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks, "gpu_launches": r["launches"], "roofline": roofline,
         "sweep_only": {"value": world * w.links / (r["sweep_ms"] * 1e-3), "unit": UNIT, "ms_per_sweep": r["sweep_ms"]},
         "init_ms": r["init_ms"], "plaquette_last": r["plaquette_last"], "polyakov_last": r["polyakov_last"],
+        "su2_run": {"value": world * w.links / (r["ms_per_step_run"] * 1e-3), "unit": UNIT,
+                    "ms_per_step": r["ms_per_step_run"],
+                    "what": "the same steps as one su2_run call (captured CUDA graph replayed), timed right after"},
     }
 
     if not args.headline_only and rank == 0:
@@ -430,6 +448,7 @@ def main():
                 "note": ("lattice %d MiB: L2-resident, HBM peak is not its bound" % lattice_mib) if lattice_mib <= 126
                 else ("lattice %d MiB > L2" % lattice_mib),
                 "plaquette_last": rr["plaquette_last"],
+                "su2_run_ms_per_step": rr["ms_per_step_run"],
             }
         line["workloads"] = others
         line["e2e"] = time_e2e(pkg, torch, w, prec, args.beta, args.e2e_steps, 1, args.seed)

@@ -135,6 +135,17 @@ SU2_API int su2_measure_async(su2_lattice* lat, double* dev_out, size_t index);
 SU2_API int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_t sweep_idx, double* dev_out,
                                        size_t index, void* event_after_sweep);
 
+/* The paper's whole loop in one call (N iterations of heat bath + plaquette):
+ * n_steps times { su2_heatbath_sweep_measure(beta, sweep_idx0 + i) } with the results of step i
+ * at dev_out[2*i] (mean plaquette) and dev_out[2*i+1] (Polyakov loop); dev_out [device] holds
+ * 2*n_steps doubles. One step is captured once per handle as a CUDA graph (11 kernels, the
+ * sub-steps chained by programmatic dependent launch) and replayed; sweep index, 1/beta and the
+ * output slot live in device memory, so no kernel parameter changes between replays
+ * (DESIGN.md 6.6). Same links and observables as the step-by-step calls, bit for bit.
+ * Runs on a private stream ordered after, and joined back into, the handle's stream.
+ * Asynchronous. Errors: SU2_EARG (beta, NULL dev_out), SU2_ESTATE, SU2_ECUDA. */
+SU2_API int su2_run(su2_lattice* lat, double beta, uint32_t sweep_idx0, uint32_t n_steps, double* dev_out);
+
 /* NEXT-1 (eq. 3): on-axis Polyakov-loop correlator
  * C(r) = < l(x) l(x + r e_i) >, averaged over all spatial x and the 3 spatial axes i,
  * r = 1..rmax (rmax <= min spatial extent / 2), l(x) = 1/2 Tr L(x) (real in SU(2)).

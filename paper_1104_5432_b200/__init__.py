@@ -35,6 +35,7 @@ _SIGNATURES = {
     "su2_heatbath_substep": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32, C.c_int, C.c_int]),
     "su2_heatbath_sweep_measure": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32, C.c_void_p, C.c_size_t,
                                              C.c_void_p]),
+    "su2_run": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32, C.c_uint32, C.c_void_p]),
     "su2_mean_plaquette": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "su2_polyakov_loop": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "su2_measure": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
@@ -128,6 +129,10 @@ def su2_heatbath_substep(h, beta, sweep_idx, mu, parity):
 def su2_heatbath_sweep_measure(h, beta, sweep_idx, dev_out_ptr, index, event_after_sweep=0):
     _check(lib().su2_heatbath_sweep_measure(h, beta, sweep_idx, C.c_void_p(dev_out_ptr), index,
                                             C.c_void_p(event_after_sweep)), h)
+
+
+def su2_run(h, beta, sweep_idx0, n_steps, dev_out_ptr):
+    _check(lib().su2_run(h, beta, sweep_idx0, n_steps, C.c_void_p(dev_out_ptr)), h)
 
 
 def su2_mean_plaquette(h):
@@ -227,6 +232,11 @@ class Lattice:
         """dev_out: torch float64 device tensor; event_after_sweep: a recorded-once torch.cuda.Event."""
         ev = event_after_sweep.cuda_event if event_after_sweep is not None else 0
         su2_heatbath_sweep_measure(self.h, beta, sweep_idx, dev_out.data_ptr(), index, ev)
+
+    def run(self, beta, sweep_idx0, n_steps, dev_out):
+        """n_steps x (sweep + plaquette + Polyakov loop); dev_out: float64 device tensor, 2*n_steps."""
+        assert dev_out.numel() >= 2 * n_steps
+        su2_run(self.h, beta, sweep_idx0, n_steps, dev_out.data_ptr())
 
     def substep(self, beta, sweep_idx, mu, parity):
         su2_heatbath_substep(self.h, beta, sweep_idx, mu, parity)

@@ -25,6 +25,12 @@ struct su2_lattice {
     int last_substep;  // 2*mu+parity of the heat-bath sub-step that was the LAST work enqueued by this
                        // handle, else -1: decides whether the next sub-step may overlap it
     bool pdl;          // programmatic dependent launch enabled (SU2HB_NO_PDL=1 disables; A/B timing only)
+    // su2_run: one step captured as a CUDA graph, replayed on a private stream
+    cudaStream_t run_stream;
+    cudaEvent_t run_ev_in, run_ev_out;
+    cudaGraphExec_t run_exec;
+    bool run_graphs;   // SU2HB_NO_GRAPH=1 disables (A/B timing only)
+    void* stage;       // canonical-order staging buffer of su2_get_links / su2_set_links (lazy, kept)
     int sticky;  // sticky error code
     char msg[256];
 };
@@ -56,12 +62,14 @@ static int fail(su2_lattice* lat, int code, const char* what, cudaError_t ce = c
 // launch sub-step (mu, parity); it may overlap the tail of the previous launch only if
 // that was its canonical predecessor [R4] on this handle
 static void enqueue_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, int mu, int parity,
-                            double* epart = nullptr)
+                            double* epart = nullptr, const RunState* state = nullptr, cudaStream_t st = nullptr,
+                            bool allow_overlap = true)
 {
     const int idx = 2 * mu + parity;
-    const bool overlap = lat->pdl && lat->last_substep == (idx + 7) % 8;
+    const bool overlap = allow_overlap && lat->pdl && lat->last_substep == (idx + 7) % 8;
+    if (!state) st = lat->stream;
     lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, parity, beta, lat->seed,
-                                             sweep_idx, lat->sc.err, epart, overlap, lat->stream);
+                                             sweep_idx, lat->sc.err, epart, state, overlap, st);
     lat->last_substep = idx;
 }
 
@@ -112,6 +120,8 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
     {
         const char* e = getenv("SU2HB_NO_PDL");
         lat->pdl = !(e && e[0] == '1');
+        e = getenv("SU2HB_NO_GRAPH");
+        lat->run_graphs = !(e && e[0] == '1');
     }
     lat->stream = (cudaStream_t)stream;
     lat->owns_links = !external;
@@ -125,6 +135,7 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.epart, 3 * heatbath_ctas(g) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.field, v3 * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.out, (2 + kMaxR) * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.state, sizeof(RunState));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.err, sizeof(int));
     if (ce == cudaSuccess) ce = cudaMemset(lat->sc.err, 0, sizeof(int));
     if (ce != cudaSuccess) {
@@ -156,7 +167,13 @@ extern "C" int su2_lattice_destroy(su2_lattice* lat)
     if (lat->sc.epart) cudaFree(lat->sc.epart);
     if (lat->sc.field) cudaFree(lat->sc.field);
     if (lat->sc.out) cudaFree(lat->sc.out);
+    if (lat->stage) cudaFree(lat->stage);
     if (lat->sc.err) cudaFree(lat->sc.err);
+    if (lat->sc.state) cudaFree(lat->sc.state);
+    if (lat->run_exec) cudaGraphExecDestroy(lat->run_exec);
+    if (lat->run_ev_in) cudaEventDestroy(lat->run_ev_in);
+    if (lat->run_ev_out) cudaEventDestroy(lat->run_ev_out);
+    if (lat->run_stream) cudaStreamDestroy(lat->run_stream);
     delete lat;
     return SU2_OK;
 }
@@ -234,6 +251,78 @@ extern "C" int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_
     lat->launches +=
         launch_polyakov(lat->links, lat->g, lat->precision, lat->sc, dev_out + 2 * index + 1, lat->stream);
     CK(lat, cudaGetLastError());
+    return SU2_OK;
+}
+
+// one step of su2_run on stream `st`, every per-step quantity read from the device RunState
+static void enqueue_run_step(su2_lattice* lat, cudaStream_t st, bool allow_overlap)
+{
+    const size_t ctas = heatbath_ctas(lat->g);
+    lat->last_substep = -1;
+    for (int mu = 0; mu < 4; ++mu)
+        for (int p = 0; p < 2; ++p)
+            enqueue_substep(lat, 1.0, 0u, mu, p, (p == 1 && mu >= 1) ? lat->sc.epart + (mu - 1) * ctas : nullptr,
+                            lat->sc.state, st, allow_overlap);
+    lat->last_substep = -1;
+    lat->launches += launch_final_sum_state(lat->sc.epart, 3 * ctas, 1.0 / (6.0 * 2.0 * (double)lat->g.vh),
+                                            lat->sc.state, 0, false, st);
+    size_t np = 0;
+    lat->launches += launch_polyakov_partials(lat->links, lat->g, lat->precision, lat->sc, &np, st);
+    const double v3 = (double)lat->g.n[0] * lat->g.n[1] * lat->g.n[2];
+    lat->launches += launch_final_sum_state(lat->sc.partials, np, 1.0 / v3, lat->sc.state, 1, true, st);
+}
+
+// capture one step into an executable graph; with programmatic edges first, without if the
+// driver refuses them
+static bool build_run_graph(su2_lattice* lat)
+{
+    for (int attempt = 0; attempt < 2 && !lat->run_exec; ++attempt) {
+        const bool overlap = attempt == 0;
+        const uint64_t launches0 = lat->launches;
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(lat->run_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
+        enqueue_run_step(lat, lat->run_stream, overlap);
+        cudaError_t ce = cudaStreamEndCapture(lat->run_stream, &graph);
+        lat->launches = launches0;  // captured, not launched
+        if (ce == cudaSuccess && graph) ce = cudaGraphInstantiate(&lat->run_exec, graph, 0);
+        if (graph) cudaGraphDestroy(graph);
+        if (ce != cudaSuccess) {
+            lat->run_exec = nullptr;
+            cudaGetLastError();
+        }
+    }
+    return lat->run_exec != nullptr;
+}
+
+extern "C" int su2_run(su2_lattice* lat, double beta, uint32_t sweep_idx0, uint32_t n_steps, double* dev_out)
+{
+    ENTER(lat);
+    NOT_A_SUBSTEP(lat);
+    if (int rc = check_beta(lat, beta)) return rc;
+    if (!dev_out && n_steps) return fail(lat, SU2_EARG, "su2_run: NULL dev_out");
+    if (n_steps == 0) return SU2_OK;
+    if (!lat->run_stream) {
+        CK(lat, cudaStreamCreateWithFlags(&lat->run_stream, cudaStreamNonBlocking));
+        CK(lat, cudaEventCreateWithFlags(&lat->run_ev_in, cudaEventDisableTiming));
+        CK(lat, cudaEventCreateWithFlags(&lat->run_ev_out, cudaEventDisableTiming));
+    }
+    // the private stream continues the handle's stream and hands back to it
+    CK(lat, cudaEventRecord(lat->run_ev_in, lat->stream));
+    CK(lat, cudaStreamWaitEvent(lat->run_stream, lat->run_ev_in, 0));
+    lat->launches += launch_set_run_state(lat->sc.state, 1.0 / beta, dev_out, sweep_idx0, 0u, lat->run_stream);
+    const bool graphs = lat->run_graphs && (lat->run_exec || build_run_graph(lat));
+    const uint64_t per_step = 8 + 3;
+    for (uint32_t i = 0; i < n_steps; ++i) {
+        if (graphs) {
+            CK(lat, cudaGraphLaunch(lat->run_exec, lat->run_stream));
+            lat->launches += per_step;
+        } else {
+            enqueue_run_step(lat, lat->run_stream, true);
+        }
+    }
+    CK(lat, cudaGetLastError());
+    CK(lat, cudaEventRecord(lat->run_ev_out, lat->run_stream));
+    CK(lat, cudaStreamWaitEvent(lat->stream, lat->run_ev_out, 0));
     return SU2_OK;
 }
 
@@ -321,16 +410,16 @@ extern "C" int su2_get_links(su2_lattice* lat, void* host_dst, size_t bytes)
     const size_t need = su2_lattice_bytes(g.n[0], g.n[1], g.n[2], g.n[3], lat->precision);
     if (!host_dst || bytes != need) return fail(lat, SU2_EARG, "su2_get_links: bad buffer");
     if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
-    void* stage = nullptr;
-    if (cudaMalloc(&stage, need) != cudaSuccess) {
+    if (!lat->stage && cudaMalloc(&lat->stage, need) != cudaSuccess) {
         cudaGetLastError();
+        lat->stage = nullptr;
         return fail(lat, SU2_EALLOC, "su2_get_links: staging buffer");
     }
+    void* stage = lat->stage;
     lat->launches += launch_to_canonical(lat->links, stage, g, lat->precision, lat->stream);
     cudaError_t ce = cudaGetLastError();
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(host_dst, stage, need, cudaMemcpyDeviceToHost, lat->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(lat->stream);
-    cudaFree(stage);
     if (ce != cudaSuccess) return fail(lat, SU2_ECUDA, "su2_get_links", ce);
     return SU2_OK;
 }
@@ -342,18 +431,18 @@ extern "C" int su2_set_links(su2_lattice* lat, const void* host_src, size_t byte
     const Geom& g = lat->g;
     const size_t need = su2_lattice_bytes(g.n[0], g.n[1], g.n[2], g.n[3], lat->precision);
     if (!host_src || bytes != need) return fail(lat, SU2_EARG, "su2_set_links: bad buffer");
-    void* stage = nullptr;
-    if (cudaMalloc(&stage, need) != cudaSuccess) {
+    if (!lat->stage && cudaMalloc(&lat->stage, need) != cudaSuccess) {
         cudaGetLastError();
+        lat->stage = nullptr;
         return fail(lat, SU2_EALLOC, "su2_set_links: staging buffer");
     }
+    void* stage = lat->stage;
     cudaError_t ce = cudaMemcpyAsync(stage, host_src, need, cudaMemcpyHostToDevice, lat->stream);
     if (ce == cudaSuccess) {
         lat->launches += launch_to_device_layout(stage, lat->links, g, lat->precision, lat->stream);
         ce = cudaGetLastError();
     }
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(lat->stream);
-    cudaFree(stage);
     if (ce != cudaSuccess) return fail(lat, SU2_ECUDA, "su2_set_links", ce);
     lat->initialised = true;
     return SU2_OK;

@@ -334,6 +334,29 @@ struct M<double> {
     static __device__ __forceinline__ double tiny() { return 1e-30; }
 };
 
+// Device-resident loop state of su2_run: a captured CUDA graph of one
+// step is replayed n times without touching its kernel parameters, so what changes from
+// step to step lives here. Written by set_run_state_kernel and advanced by the last
+// kernel of every step.
+struct RunState {
+    double inv_beta;
+    double* out;      // [device] 2 doubles per step
+    uint32_t sweep;   // sweep_idx of the current step
+    uint32_t index;   // step number: results go to out[2*index], out[2*index+1]
+};
+__device__ __forceinline__ uint32_t ld_cg_u32(const uint32_t* p)
+{
+    uint32_t v;
+    asm volatile("ld.global.cg.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ double ld_cg_f64(const double* p)
+{
+    double v;
+    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // per-launch constants of the heat-bath kernels. The array bases are resolved on the
 // host so that a link address is base + 16*(32-bit index): one IMAD.WIDE per load.
 template <typename Real>
@@ -343,6 +366,7 @@ struct __align__(16) HbParams {
     const typename LinkPtr<Real>::type* oppo[4];  // U_nu on the other parity
     typename LinkPtr<Real>::type* out;            // U_mu on the parity being updated
     double* epart;                                // fused plaquette: one partial per CTA (MEAS kernels)
+    const RunState* state;                        // non-null inside su2_run: sweep and 1/beta come from here
     Real inv_beta;
     uint32_t sweep;
 };

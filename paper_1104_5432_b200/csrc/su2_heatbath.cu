@@ -48,6 +48,13 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     grid_dep_wait();    // the preceding kernel of the stream has finished and flushed
     grid_dep_launch();  // ... so the next one may be scheduled behind this CTA
 
+    uint32_t sweep = hp.sweep;
+    Real inv_beta = hp.inv_beta;
+    if (hp.state) {  // su2_run: the captured graph's parameters are frozen, the loop state is not
+        sweep = ld_cg_u32(&hp.state->sweep);
+        inv_beta = (Real)ld_cg_f64(&hp.state->inv_beta);
+    }
+
     Quat<Real> a[3], b[3], cc[3], a2[3], b2[3], c2[3];
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
@@ -67,7 +74,7 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     // [R5] counter = (s, sweep, (p<<2)|mu, n); the n = 0 draw does not depend on the links
     const uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
     const uint32_t tag = ((uint32_t)P << 2) | (uint32_t)MU;
-    const Words wd = philox_keyed(s, hp.sweep, tag, 0u, hp.rk);
+    const Words wd = philox_keyed(s, sweep, tag, 0u, hp.rk);
 
     // [R3] staple sum, nu ascending, forward then backward, products left to right;
     // the second product of every term accumulates straight into v (FMA chains).
@@ -85,12 +92,12 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
         u = haar_from_words<Real>(wd);
     } else {
         const Real rk = M<Real>::rsqrt(k2);       // 1/k
-        const Real inv_alpha = rk * hp.inv_beta;  // 1/(beta k)
+        const Real inv_alpha = rk * inv_beta;  // 1/(beta k)
         // [R6] Kennedy-Pendleton
         Real delta = 0;
         uint32_t n = 1;
         for (;;) {
-            const Words w = philox_keyed(s, hp.sweep, tag, n, hp.rk);
+            const Words w = philox_keyed(s, sweep, tag, n, hp.rk);
             delta = M<Real>::kp_delta(w, inv_alpha);
             const Real Rppp = M<Real>::uniform(w.w3);
             if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) {
@@ -244,7 +251,7 @@ static void launch_ex(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStrea
 
 template <typename Real, int MU, int P, bool MEAS>
 static int launch_substep_t(void* links, const Geom& g, double beta, uint64_t seed, uint32_t sweep, int* err,
-                            double* epart, bool overlap, cudaStream_t st)
+                            double* epart, const RunState* state, bool overlap, cudaStream_t st)
 {
     typedef typename LinkPtr<Real>::type L;
     HbParams<Real> hp;
@@ -257,6 +264,7 @@ static int launch_substep_t(void* links, const Geom& g, double beta, uint64_t se
     }
     hp.out = (L*)links + (size_t)(P * 4 + MU) * g.vh;
     hp.epart = epart;
+    hp.state = state;
     const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
     if (g.tile == 0) {
         launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>,
@@ -282,24 +290,25 @@ size_t heatbath_ctas(const Geom& g)
 
 template <typename Real>
 static int launch_substep_p(void* links, const Geom& g, int mu, int parity, double beta, uint64_t seed,
-                            uint32_t sweep, int* err, double* epart, bool overlap, cudaStream_t st)
+                            uint32_t sweep, int* err, double* epart, const RunState* state, bool overlap,
+                            cudaStream_t st)
 {
     if (epart && parity == 1 && mu >= 1) {  // the three measuring kernels
         switch (mu) {
-            case 1: return launch_substep_t<Real, 1, 1, true>(links, g, beta, seed, sweep, err, epart, overlap, st);
-            case 2: return launch_substep_t<Real, 2, 1, true>(links, g, beta, seed, sweep, err, epart, overlap, st);
-            default: return launch_substep_t<Real, 3, 1, true>(links, g, beta, seed, sweep, err, epart, overlap, st);
+            case 1: return launch_substep_t<Real, 1, 1, true>(links, g, beta, seed, sweep, err, epart, state, overlap, st);
+            case 2: return launch_substep_t<Real, 2, 1, true>(links, g, beta, seed, sweep, err, epart, state, overlap, st);
+            default: return launch_substep_t<Real, 3, 1, true>(links, g, beta, seed, sweep, err, epart, state, overlap, st);
         }
     }
     switch (mu * 2 + parity) {
-        case 0: return launch_substep_t<Real, 0, 0, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
-        case 1: return launch_substep_t<Real, 0, 1, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
-        case 2: return launch_substep_t<Real, 1, 0, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
-        case 3: return launch_substep_t<Real, 1, 1, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
-        case 4: return launch_substep_t<Real, 2, 0, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
-        case 5: return launch_substep_t<Real, 2, 1, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
-        case 6: return launch_substep_t<Real, 3, 0, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
-        default: return launch_substep_t<Real, 3, 1, false>(links, g, beta, seed, sweep, err, nullptr, overlap, st);
+        case 0: return launch_substep_t<Real, 0, 0, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
+        case 1: return launch_substep_t<Real, 0, 1, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
+        case 2: return launch_substep_t<Real, 1, 0, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
+        case 3: return launch_substep_t<Real, 1, 1, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
+        case 4: return launch_substep_t<Real, 2, 0, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
+        case 5: return launch_substep_t<Real, 2, 1, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
+        case 6: return launch_substep_t<Real, 3, 0, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
+        default: return launch_substep_t<Real, 3, 1, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
     }
 }
 
@@ -308,11 +317,12 @@ static int launch_substep_p(void* links, const Geom& g, int mu, int parity, doub
 // where the sub-steps (mu >= 1, parity 1) store their heatbath_ctas(g) fused-plaquette
 // partials; ignored by the other sub-steps.
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
-                            uint64_t seed, uint32_t sweep, int* err, double* epart, bool overlap, cudaStream_t st)
+                            uint64_t seed, uint32_t sweep, int* err, double* epart, const RunState* state,
+                            bool overlap, cudaStream_t st)
 {
     return precision == 32
-               ? launch_substep_p<float>(links, g, mu, parity, beta, seed, sweep, err, epart, overlap, st)
-               : launch_substep_p<double>(links, g, mu, parity, beta, seed, sweep, err, epart, overlap, st);
+               ? launch_substep_p<float>(links, g, mu, parity, beta, seed, sweep, err, epart, state, overlap, st)
+               : launch_substep_p<double>(links, g, mu, parity, beta, seed, sweep, err, epart, state, overlap, st);
 }
 
 int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st)

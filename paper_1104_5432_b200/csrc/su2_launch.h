@@ -30,6 +30,7 @@ struct Scratch {
     double* field;      // [device] l(x) of the Polyakov kernel, V/Nt doubles
     double* out;        // [device] 2 + kMaxR doubles: plaquette, polyakov, correlator
     int* err;           // [device] sticky error flags (bit 0: KP trial cap hit)
+    RunState* state;    // [device] loop state of su2_run
 };
 constexpr int kMaxR = 128;
 
@@ -40,9 +41,18 @@ size_t partials_needed(const Geom& g);
 // each returns the number of kernels it enqueued (0 on launch failure; check cudaGetLastError)
 int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st);
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
-                            uint64_t seed, uint32_t sweep, int* err, double* epart, bool overlap, cudaStream_t st);
+                            uint64_t seed, uint32_t sweep, int* err, double* epart, const RunState* state, bool overlap,
+                            cudaStream_t st);
 size_t heatbath_ctas(const Geom& g);
 int launch_final_sum(const double* partials, size_t n, double scale, double* dev_dst, cudaStream_t st);
+// su2_run: the destination is state->out[2*state->index + slot]; `advance` also bumps sweep and index
+int launch_final_sum_state(const double* partials, size_t n, double scale, RunState* state, int slot, bool advance,
+                           cudaStream_t st);
+int launch_set_run_state(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index,
+                         cudaStream_t st);
+// Polyakov partials only (no final sum): used by su2_run, which sums them with launch_final_sum_state
+int launch_polyakov_partials(const void* links, const Geom& g, int precision, const Scratch& sc, size_t* n_partials,
+                             cudaStream_t st);
 int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
                      cudaStream_t st);
 int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,

@@ -263,14 +263,51 @@ int launch_plaquette(const void* links, const Geom& g, int precision, const Scra
     return 2;
 }
 
+// su2_run variants: destination and loop counters live in the device RunState
+__global__ void __launch_bounds__(1024)
+    final_sum_state_kernel(const double* __restrict__ partials, size_t n, double scale, RunState* __restrict__ state,
+                           int slot, int advance)
+{
+    __shared__ double red[32];
+    double acc = 0.0;
+    for (size_t i = threadIdx.x; i < n; i += 1024) acc += partials[i];
+    const double tot = block_sum(acc, red);
+    if (threadIdx.x == 0) {
+        state->out[2 * (size_t)state->index + slot] = tot * scale;
+        if (advance) {
+            state->sweep += 1u;
+            state->index += 1u;
+        }
+    }
+}
+__global__ void set_run_state_kernel(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index)
+{
+    state->inv_beta = inv_beta;
+    state->out = out;
+    state->sweep = sweep;
+    state->index = index;
+}
+int launch_final_sum_state(const double* partials, size_t n, double scale, RunState* state, int slot, bool advance,
+                           cudaStream_t st)
+{
+    final_sum_state_kernel<<<1, 1024, 0, st>>>(partials, n, scale, state, slot, advance ? 1 : 0);
+    return 1;
+}
+int launch_set_run_state(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index,
+                         cudaStream_t st)
+{
+    set_run_state_kernel<<<1, 1, 0, st>>>(state, inv_beta, out, sweep, index);
+    return 1;
+}
+
 int launch_final_sum(const double* partials, size_t n, double scale, double* dev_dst, cudaStream_t st)
 {
     final_sum_kernel<<<1, 1024, 0, st>>>(partials, n, scale, dev_dst);
     return 1;
 }
 
-int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
-                    cudaStream_t st)
+int launch_polyakov_partials(const void* links, const Geom& g, int precision, const Scratch& sc, size_t* n_partials,
+                             cudaStream_t st)
 {
     const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
     const unsigned grid = blocks_for(v3);
@@ -278,7 +315,17 @@ int launch_polyakov(const void* links, const Geom& g, int precision, const Scrat
         polyakov_kernel<float><<<grid, kBlock, 0, st>>>((const float4*)links, g, sc.field, sc.partials);
     else
         polyakov_kernel<double><<<grid, kBlock, 0, st>>>((const double4a*)links, g, sc.field, sc.partials);
-    final_sum_kernel<<<1, 1024, 0, st>>>(sc.partials, grid, 1.0 / (double)v3, dev_dst);
+    *n_partials = grid;
+    return 1;
+}
+
+int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
+                    cudaStream_t st)
+{
+    size_t n = 0;
+    launch_polyakov_partials(links, g, precision, sc, &n, st);
+    const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
+    final_sum_kernel<<<1, 1024, 0, st>>>(sc.partials, n, 1.0 / (double)v3, dev_dst);
     return 2;
 }
 

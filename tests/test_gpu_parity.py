@@ -391,3 +391,35 @@ def test_sweep_measure_fused_plaquette_matches_oracle_and_standalone_kernel(pkg,
         assert abs(P - a.mean_plaquette()) < (1e-13 if prec == 64 else 2e-7)
     a.close()
     b.close()
+
+
+@pytest.mark.parametrize("graphs", ["1", "0"])
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", [(16, 8, 8, 4), (32, 4, 4, 2), (8, 8, 8, 8), (6, 4, 10, 2)])
+def test_run_equals_step_by_step_calls_bitwise(pkg, dims, prec, graphs, monkeypatch):
+    """su2_run (captured CUDA graph replayed n times, loop state in device memory) against n
+    su2_heatbath_sweep_measure calls: identical links and observables; also with the graph
+    disabled (direct launches reading the same device state)."""
+    import torch
+    monkeypatch.setenv("SU2HB_NO_GRAPH", "0" if graphs == "1" else "1")
+    n = 7
+    a, b = pkg.Lattice(dims, prec), pkg.Lattice(dims, prec)
+    oa = torch.zeros(2 * n, dtype=torch.float64, device="cuda")
+    ob = torch.zeros(2 * n, dtype=torch.float64, device="cuda")
+    for lat in (a, b):
+        lat.init("hot", 21)
+    for i in range(n):
+        a.sweep_measure(2.4, 10 + i, oa, i)
+    b.run(2.4, 10, 3, ob)          # two calls: the second replays the cached graph
+    b.run(2.4, 13, n - 3, ob[6:])
+    assert (a.get_links() == b.get_links()).all()
+    assert (oa.cpu() == ob.cpu()).all()
+    # and the oracle agrees with the whole chain in fp64 (no flips expected)
+    if prec == 64:
+        L = oracle.init(dims, "hot", 21, "f64")
+        for i in range(n):
+            oracle.heatbath_sweep(dims, L, 2.4, 21, 10 + i, "f64")
+            assert abs(float(ob[2 * i]) - oracle.mean_plaquette(dims, L, "f64")) < 1e-12
+        assert_links_match(b.get_links(), L, 64)
+    a.close()
+    b.close()
