@@ -32,30 +32,29 @@ namespace su2 {
 // touched by any later sub-step of the sweep and each of their plaquettes holds exactly
 // one odd-parity mu-link, so the three kernels (1,1), (2,1), (3,1) together sum every
 // plaquette of the final configuration exactly once.
-template <typename Real, int MU, int P, bool MEAS>
-__device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
-                                              int* __restrict__ err)
+template <typename Real>
+struct Staple18 {  // the 18 links of one staple sum, per direction nu != mu (i = 0..2)
+    Quat<Real> a[3], b[3], cc[3], a2[3], b2[3], c2[3];
+};
+struct SiteIdx {
+    int h;  // half-index of the site
+    int r;  // low bit of x
+};
+
+// neighbour addressing (row 2) and the 18 loads (row 3, first half) of one site
+template <typename Real, int MU, int P>
+__device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const HbParams<Real>& hp, Staple18<Real>& q)
 {
     typedef typename LinkPtr<Real>::type L;
     constexpr int DEP_NU = (P == 0) ? (MU + 3) % 4 : -1;
     constexpr bool DEP_MU = (P == 1);
-    const int r = (c.y + c.z + c.t + P) & 1;
-    const int h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
-    const Nbr d = neighbours(g, c, r);
+    SiteIdx ix;
+    ix.r = (c.y + c.z + c.t + P) & 1;
+    ix.h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
+    const int h = ix.h;
+    const Nbr d = neighbours(g, c, ix.r);
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
     const uint32_t h_up = (uint32_t)(h + d.up[MU]);
-
-    grid_dep_wait();    // the preceding kernel of the stream has finished and flushed
-    grid_dep_launch();  // ... so the next one may be scheduled behind this CTA
-
-    uint32_t sweep = hp.sweep;
-    Real inv_beta = hp.inv_beta;
-    if (hp.state) {  // su2_run: the captured graph's parameters are frozen, the loop state is not
-        sweep = ld_cg_u32(&hp.state->sweep);
-        inv_beta = (Real)ld_cg_f64(&hp.state->inv_beta);
-    }
-
-    Quat<Real> a[3], b[3], cc[3], a2[3], b2[3], c2[3];
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         const int nu = i + (i >= MU ? 1 : 0);
@@ -63,14 +62,37 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
         const L* o_nu = hp.oppo[nu];
         const uint32_t h_dn = (uint32_t)(h + d.dn[nu]);
         const uint32_t h_upnu = (uint32_t)(h + d.up[nu]);
-        a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
-        b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
-        cc[i] = ldq(s_nu + (uint32_t)h);                                  // U_nu(x)
-        a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));             // U_nu(x+mu-nu)
-        b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
-        c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
+        q.a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
+        q.b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
+        q.cc[i] = ldq(s_nu + (uint32_t)h);                                  // U_nu(x)
+        q.a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));             // U_nu(x+mu-nu)
+        q.b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
+        q.c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
     }
+    return ix;
+}
 
+// rows 3 (products) to 6: staple sum, Philox, Kennedy-Pendleton, compose, store
+template <typename Real, int MU, int P, bool MEAS>
+__device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteIdx ix, uint32_t sweep, Real inv_beta,
+                                            const HbParams<Real>& hp, int* __restrict__ err)
+{
+    const Quat<Real>*a = q.a, *b = q.b, *cc = q.cc, *a2 = q.a2, *b2 = q.b2, *c2 = q.c2;
+    const int h = ix.h, r = ix.r;
+#ifdef HB_PROBE_MEMONLY  // tuning probe (never in the product build): the 18 loads, a sum, the store
+    {
+        Quat<Real> sacc = {0, 0, 0, 0};
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            sacc.a0 += a[i].a0 + b[i].a0 + cc[i].a0 + a2[i].a0 + b2[i].a0 + c2[i].a0;
+            sacc.a1 += a[i].a1 + b[i].a1 + cc[i].a1 + a2[i].a1 + b2[i].a1 + c2[i].a1;
+            sacc.a2 += a[i].a2 + b[i].a2 + cc[i].a2 + a2[i].a2 + b2[i].a2 + c2[i].a2;
+            sacc.a3 += a[i].a3 + b[i].a3 + cc[i].a3 + a2[i].a3 + b2[i].a3 + c2[i].a3;
+        }
+        stq(hp.out + (uint32_t)h, sacc);
+        return (Real)0;
+    }
+#endif
     // [R5] counter = (s, sweep, (p<<2)|mu, n); the n = 0 draw does not depend on the links
     const uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
     const uint32_t tag = ((uint32_t)P << 2) | (uint32_t)MU;
@@ -125,6 +147,31 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     u.a0 *= inv; u.a1 *= inv; u.a2 *= inv; u.a3 *= inv;
     stq(hp.out + (uint32_t)h, u);
     return MEAS ? u.a0 * w.a0 - u.a1 * w.a1 - u.a2 * w.a2 - u.a3 * w.a3 : (Real)0;  // 1/2 Tr(U' w)
+}
+
+template <typename Real>
+__device__ __forceinline__ void run_state(const HbParams<Real>& hp, uint32_t& sweep, Real& inv_beta)
+{
+    sweep = hp.sweep;
+    inv_beta = hp.inv_beta;
+    if (hp.state) {  // su2_run: the captured graph's parameters are frozen, the loop state is not
+        sweep = ld_cg_u32(&hp.state->sweep);
+        inv_beta = (Real)ld_cg_f64(&hp.state->inv_beta);
+    }
+}
+
+template <typename Real, int MU, int P, bool MEAS>
+__device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
+                                              int* __restrict__ err)
+{
+    grid_dep_wait();    // the preceding kernel of the stream has finished and flushed
+    grid_dep_launch();  // ... so the next one may be scheduled behind this CTA
+    uint32_t sweep;
+    Real inv_beta;
+    run_state(hp, sweep, inv_beta);
+    Staple18<Real> q;
+    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q);
+    return update_link<Real, MU, P, MEAS>(q, ix, sweep, inv_beta, hp, err);
 }
 
 // Resident CTAs per SM that ptxas must allow: this is the register budget that lets it
