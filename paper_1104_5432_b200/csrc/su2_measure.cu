@@ -154,6 +154,52 @@ __global__ void __launch_bounds__(kBlock)
     if (threadIdx.x == 0) partials[blockIdx.x] = tot;
 }
 
+// Long time extents: S threads per spatial site, each the ordered product of N_t/S
+// consecutive time links; the S partial products are multiplied in order through shared
+// memory. S = 1 above is the plain loop; S is fixed by N_t, so a lattice always gives the
+// same bits. (32^4: the one-thread-per-site loop is 32 dependent loads deep on only 128 CTAs.)
+template <typename Real, int S>
+__global__ void __launch_bounds__(kBlock)
+    polyakov_split_kernel(const typename LinkPtr<Real>::type* __restrict__ links, const Geom g,
+                          double* __restrict__ field, double* __restrict__ partials)
+{
+    typedef typename LinkPtr<Real>::type L;
+    constexpr int SITES = kBlock / S;
+    __shared__ double red[kBlock / 32];
+    __shared__ Quat<Real> part[S][SITES];
+    const uint32_t v3 = (uint32_t)g.n[0] * (uint32_t)g.n[1] * (uint32_t)g.n[2];
+    const int seg = threadIdx.x / SITES, lane = threadIdx.x % SITES;
+    const uint32_t s3 = blockIdx.x * (uint32_t)SITES + lane;
+    const int len = g.n[3] / S, t0 = seg * len;
+    if (s3 < v3) {
+        const uint32_t x = s3 % (uint32_t)g.n[0];
+        const uint32_t q = s3 / (uint32_t)g.n[0];
+        const uint32_t y = q % (uint32_t)g.n[1], z = q / (uint32_t)g.n[1];
+        const int p0 = (int)((x + y + z) & 1u);
+        const size_t vh = g.vh;
+        const L* a0 = links + (size_t)(p0 * 4 + 3) * vh + (s3 >> 1);        // even t
+        const L* a1 = links + (size_t)((1 - p0) * 4 + 3) * vh + (s3 >> 1);  // odd t
+        Quat<Real> prod = ldq(((t0 & 1) ? a1 : a0) + (size_t)t0 * (size_t)g.st);
+#pragma unroll 4
+        for (int t = t0 + 1; t < t0 + len; ++t) {
+            const Quat<Real> u = ldq(((t & 1) ? a1 : a0) + (size_t)t * (size_t)g.st);
+            prod = qmul<false, false>(prod, u);
+        }
+        part[seg][lane] = prod;
+    }
+    __syncthreads();
+    double val = 0.0;
+    if (seg == 0 && s3 < v3) {
+        Quat<Real> prod = part[0][lane];
+#pragma unroll
+        for (int k = 1; k < S; ++k) prod = qmul<false, false>(prod, part[k][lane]);
+        val = (double)prod.a0;
+        if (field) field[s3] = val;
+    }
+    const double tot = block_sum(val, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+}
+
 // ------------------------------------------------------------------ correlator (NEXT-1)
 // C(r) = 1/(3 V3) sum_x sum_{i=x,y,z} l(x) l(x + r e_i);  grid.y = r-1
 __global__ void __launch_bounds__(kBlock)
@@ -306,16 +352,32 @@ int launch_final_sum(const double* partials, size_t n, double scale, double* dev
     return 1;
 }
 
+template <typename Real>
+static unsigned launch_polyakov_t(const void* links, const Geom& g, const Scratch& sc, cudaStream_t st)
+{
+    typedef typename LinkPtr<Real>::type L;
+    const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
+    const int nt = g.n[3];
+    if (nt >= 16 && nt % 4 == 0) {
+        const unsigned grid = (unsigned)((v3 + kBlock / 4 - 1) / (kBlock / 4));
+        polyakov_split_kernel<Real, 4><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.field, sc.partials);
+        return grid;
+    }
+    if (nt >= 8 && nt % 2 == 0) {
+        const unsigned grid = (unsigned)((v3 + kBlock / 2 - 1) / (kBlock / 2));
+        polyakov_split_kernel<Real, 2><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.field, sc.partials);
+        return grid;
+    }
+    const unsigned grid = blocks_for(v3);
+    polyakov_kernel<Real><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.field, sc.partials);
+    return grid;
+}
+
 int launch_polyakov_partials(const void* links, const Geom& g, int precision, const Scratch& sc, size_t* n_partials,
                              cudaStream_t st)
 {
-    const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
-    const unsigned grid = blocks_for(v3);
-    if (precision == 32)
-        polyakov_kernel<float><<<grid, kBlock, 0, st>>>((const float4*)links, g, sc.field, sc.partials);
-    else
-        polyakov_kernel<double><<<grid, kBlock, 0, st>>>((const double4a*)links, g, sc.field, sc.partials);
-    *n_partials = grid;
+    *n_partials = precision == 32 ? launch_polyakov_t<float>(links, g, sc, st)
+                                  : launch_polyakov_t<double>(links, g, sc, st);
     return 1;
 }
 
