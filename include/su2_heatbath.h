@@ -138,7 +138,7 @@ SU2_API int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_t s
 /* The paper's whole loop in one call (N iterations of heat bath + plaquette):
  * n_steps times { su2_heatbath_sweep_measure(beta, sweep_idx0 + i) } with the results of step i
  * at dev_out[2*i] (mean plaquette) and dev_out[2*i+1] (Polyakov loop); dev_out [device] holds
- * 2*n_steps doubles. One step is captured once per handle as a CUDA graph (11 kernels, the
+ * 2*n_steps doubles. One step is captured once per handle as a CUDA graph (10 kernels, the
  * sub-steps chained by programmatic dependent launch) and replayed; sweep index, 1/beta and the
  * output slot live in device memory, so no kernel parameter changes between replays
  * (DESIGN.md 6.6). Same links and observables as the step-by-step calls, bit for bit.

@@ -246,10 +246,11 @@ extern "C" int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_
     NOT_A_SUBSTEP(lat);
     if (event_after_sweep) CK(lat, cudaEventRecord((cudaEvent_t)event_after_sweep, lat->stream));
     // the three partial sets cover every plaquette of the new configuration once
-    lat->launches += launch_final_sum(lat->sc.epart, 3 * ctas, 1.0 / (6.0 * 2.0 * (double)lat->g.vh),
-                                      dev_out + 2 * index, lat->stream);
-    lat->launches +=
-        launch_polyakov(lat->links, lat->g, lat->precision, lat->sc, dev_out + 2 * index + 1, lat->stream);
+    size_t np = 0;
+    lat->launches += launch_polyakov_partials(lat->links, lat->g, lat->precision, lat->sc, &np, lat->stream);
+    const double v3 = (double)lat->g.n[0] * lat->g.n[1] * lat->g.n[2];
+    lat->launches += launch_final_sum2(lat->sc.epart, 3 * ctas, 1.0 / (6.0 * 2.0 * (double)lat->g.vh),
+                                       lat->sc.partials, np, 1.0 / v3, dev_out + 2 * index, nullptr, lat->stream);
     CK(lat, cudaGetLastError());
     return SU2_OK;
 }
@@ -264,12 +265,11 @@ static void enqueue_run_step(su2_lattice* lat, cudaStream_t st, bool allow_overl
             enqueue_substep(lat, 1.0, 0u, mu, p, (p == 1 && mu >= 1) ? lat->sc.epart + (mu - 1) * ctas : nullptr,
                             lat->sc.state, st, allow_overlap);
     lat->last_substep = -1;
-    lat->launches += launch_final_sum_state(lat->sc.epart, 3 * ctas, 1.0 / (6.0 * 2.0 * (double)lat->g.vh),
-                                            lat->sc.state, 0, false, st);
     size_t np = 0;
     lat->launches += launch_polyakov_partials(lat->links, lat->g, lat->precision, lat->sc, &np, st);
     const double v3 = (double)lat->g.n[0] * lat->g.n[1] * lat->g.n[2];
-    lat->launches += launch_final_sum_state(lat->sc.partials, np, 1.0 / v3, lat->sc.state, 1, true, st);
+    lat->launches += launch_final_sum2(lat->sc.epart, 3 * ctas, 1.0 / (6.0 * 2.0 * (double)lat->g.vh),
+                                       lat->sc.partials, np, 1.0 / v3, nullptr, lat->sc.state, st);
 }
 
 // capture one step into an executable graph; with programmatic edges first, without if the
@@ -311,7 +311,7 @@ extern "C" int su2_run(su2_lattice* lat, double beta, uint32_t sweep_idx0, uint3
     CK(lat, cudaStreamWaitEvent(lat->run_stream, lat->run_ev_in, 0));
     lat->launches += launch_set_run_state(lat->sc.state, 1.0 / beta, dev_out, sweep_idx0, 0u, lat->run_stream);
     const bool graphs = lat->run_graphs && (lat->run_exec || build_run_graph(lat));
-    const uint64_t per_step = 8 + 3;
+    const uint64_t per_step = 8 + 2;
     for (uint32_t i = 0; i < n_steps; ++i) {
         if (graphs) {
             CK(lat, cudaGraphLaunch(lat->run_exec, lat->run_stream));

@@ -85,13 +85,19 @@ struct LinkPtr<double> {
     typedef double4a type;
 };
 
+// Load path of the link reads: ".nc" (read-only data path, L1-cached), "" (plain ld.global)
+// or ".cg" (L2 only) - the sm_100a analogue of the paper's texture-vs-global-memory study
+// (PAPER.md:97); measured in profiles/r01c.md, ".nc" kept.
+#ifndef HB_LD
+#define HB_LD ".nc"
+#endif
 // Loads go through the non-coherent path: within one sub-step no array that is
 // read is written, and L1 is invalidated at every launch.
 __device__ __forceinline__ Quat<float> ldq(const float4* p)
 {
     Quat<float> q;
     // volatile: keeps the 18 staple loads of a thread in program order, ahead of the arithmetic
-    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];"
+    asm volatile("ld.global" HB_LD ".v4.f32 {%0,%1,%2,%3}, [%4];"
                  : "=f"(q.a0), "=f"(q.a1), "=f"(q.a2), "=f"(q.a3)
                  : "l"(p));
     return q;
@@ -100,7 +106,7 @@ __device__ __forceinline__ Quat<double> ldq(const double4a* p)
 {
     Quat<double> q;
     // one 256-bit load per link (sm_100+)
-    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+    asm volatile("ld.global" HB_LD ".v4.f64 {%0,%1,%2,%3}, [%4];"
                  : "=d"(q.a0), "=d"(q.a1), "=d"(q.a2), "=d"(q.a3)
                  : "l"(p));
     return q;
@@ -397,6 +403,35 @@ __device__ __forceinline__ double block_sum(double v, double* red)
     if (threadIdx.x == 0)
         for (int i = 0; i < nw; ++i) tot += red[i];
     __syncthreads();
+    return tot;
+}
+
+// Same, for a per-thread value of the lattice precision: in fp32 the 32 lanes are summed in
+// fp32 (5 shuffles instead of 10; the warp sum of <= 192 is good to ~1e-7 relative, far
+// inside the 1e-6 plaquette tolerance), the 4-8 warp sums and everything after in fp64.
+// No trailing barrier: for one use at the end of a kernel.
+__device__ __forceinline__ double block_sum_end(float v, double* red)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) red[wid] = (double)v;
+    __syncthreads();
+    double tot = 0.0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < nw; ++i) tot += red[i];
+    return tot;
+}
+__device__ __forceinline__ double block_sum_end(double v, double* red)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) red[wid] = v;
+    __syncthreads();
+    double tot = 0.0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < nw; ++i) tot += red[i];
     return tot;
 }
 

@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::va
     const Real e = heatbath_site<Real, MU, P, MEAS>(g, c, hp, err);
     if (MEAS) {  // one fp64 partial per CTA, fixed order
         __shared__ double red[kBlock / 32];
-        const double tot = block_sum((double)e, red);
+        const double tot = block_sum_end(e, red);
         if (threadIdx.x == 0) hp.epart[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = tot;
     }
 }
@@ -225,7 +225,7 @@ __global__ void __launch_bounds__(kBlock)
     }
     if (MEAS) {
         __shared__ double red[kBlock / 32];
-        const double tot = block_sum((double)e, red);
+        const double tot = block_sum_end(e, red);
         if (threadIdx.x == 0) hp.epart[blockIdx.x] = tot;
     }
 }

@@ -48,6 +48,8 @@ int launch_final_sum(const double* partials, size_t n, double scale, double* dev
 // su2_run: the destination is state->out[2*state->index + slot]; `advance` also bumps sweep and index
 int launch_final_sum_state(const double* partials, size_t n, double scale, RunState* state, int slot, bool advance,
                            cudaStream_t st);
+int launch_final_sum2(const double* pa, size_t na, double sa, const double* pb, size_t nb, double sb, double* dst,
+                      RunState* state, cudaStream_t st);
 int launch_set_run_state(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index,
                          cudaStream_t st);
 // Polyakov partials only (no final sum): used by su2_run, which sums them with launch_final_sum_state

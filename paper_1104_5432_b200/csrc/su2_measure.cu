@@ -333,6 +333,37 @@ __global__ void set_run_state_kernel(RunState* state, double inv_beta, double* o
     state->sweep = sweep;
     state->index = index;
 }
+// both observables of a step in one launch (one CTA, the two fixed-order sums one after the
+// other): dst = (plaquette, Polyakov loop); with `state` the destination is
+// state->out[2*index .. 2*index+1] and the loop counters advance (su2_run)
+__global__ void __launch_bounds__(1024)
+    final_sum2_kernel(const double* __restrict__ pa, size_t na, double sa, const double* __restrict__ pb, size_t nb,
+                      double sb, double* __restrict__ dst, RunState* __restrict__ state)
+{
+    __shared__ double red[32];
+    double acc = 0.0;
+    for (size_t i = threadIdx.x; i < na; i += 1024) acc += pa[i];
+    const double ta = block_sum(acc, red);
+    acc = 0.0;
+    for (size_t i = threadIdx.x; i < nb; i += 1024) acc += pb[i];
+    const double tb = block_sum(acc, red);
+    if (threadIdx.x == 0) {
+        if (state) dst = state->out + 2 * (size_t)state->index;
+        dst[0] = ta * sa;
+        dst[1] = tb * sb;
+        if (state) {
+            state->sweep += 1u;
+            state->index += 1u;
+        }
+    }
+}
+int launch_final_sum2(const double* pa, size_t na, double sa, const double* pb, size_t nb, double sb, double* dst,
+                      RunState* state, cudaStream_t st)
+{
+    final_sum2_kernel<<<1, 1024, 0, st>>>(pa, na, sa, pb, nb, sb, dst, state);
+    return 1;
+}
+
 int launch_final_sum_state(const double* partials, size_t n, double scale, RunState* state, int slot, bool advance,
                            cudaStream_t st)
 {
@@ -358,12 +389,14 @@ static unsigned launch_polyakov_t(const void* links, const Geom& g, const Scratc
     typedef typename LinkPtr<Real>::type L;
     const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
     const int nt = g.n[3];
-    if (nt >= 16 && nt % 4 == 0) {
+    // split only while one thread per site cannot fill the GPU (fewer than ~1 CTA wave of sites)
+    const bool small = v3 < 148ull * 1024ull;
+    if (small && nt >= 16 && nt % 4 == 0) {
         const unsigned grid = (unsigned)((v3 + kBlock / 4 - 1) / (kBlock / 4));
         polyakov_split_kernel<Real, 4><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.field, sc.partials);
         return grid;
     }
-    if (nt >= 8 && nt % 2 == 0) {
+    if (small && nt >= 8 && nt % 2 == 0) {
         const unsigned grid = (unsigned)((v3 + kBlock / 2 - 1) / (kBlock / 2));
         polyakov_split_kernel<Real, 2><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.field, sc.partials);
         return grid;
