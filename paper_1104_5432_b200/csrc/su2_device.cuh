@@ -8,6 +8,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "su2_math64.cuh"
+
 namespace su2 {
 
 // ---------------------------------------------------------------- geometry
@@ -291,7 +293,7 @@ struct M<float> {
         *c = -__cosf(x);
     }
     // [R6] delta of one KP trial, MUFU lg2/cos (abs. error of delta <= ~4e-7/alpha)
-    static __device__ __forceinline__ float kp_delta(const Words& w, float inv_alpha)
+    static __device__ __forceinline__ float kp_delta(const Words& w, float inv_alpha, const m64::LogEntry*)
     {
         const float cs = __cosf(angle(w.w1));  // cos(2 pi R' - pi); only its square is used
         const float g2 = fmaf(cs * cs, lg2(uniform(w.w2)), lg2(uniform(w.w0)));
@@ -322,19 +324,21 @@ struct M<double> {
     static __device__ __forceinline__ double log(double x) { return ::log(x); }
     static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
     static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
-    static __device__ __forceinline__ double rsqrt(double x) { return ::rsqrt(x); }
-    static __device__ __forceinline__ double sqrt0(double x) { return x * ::rsqrt(fmax(x, 1e-300)); }  // x >= 0
+    // su2_math64.cuh: functions specialised to the arguments of this path
+    static __device__ __forceinline__ double rsqrt(double x) { return m64::rsqrt_n(x); }  // x normal
+    static __device__ __forceinline__ double sqrt0(double x) { return x * m64::rsqrt_n(fmax(x, 1e-300)); }  // x >= 0
     static __device__ __forceinline__ double cos2pi(double x) { return cospi(2.0 * x); }
     static __device__ __forceinline__ void sincos2pi(double x, double* s, double* c) { sincospi(2.0 * x, s, c); }
     static __device__ __forceinline__ void sincos2pi_word(uint32_t w, double* s, double* c)
     {
-        sincospi(2.0 * uniform(w), s, c);
+        m64::sincos_2pi_uniform(w, s, c);
     }
-    // [R6] delta of one KP trial
-    static __device__ __forceinline__ double kp_delta(const Words& w, double inv_alpha)
+    // [R6] delta of one KP trial; `tab` = the log table in shared memory
+    static __device__ __forceinline__ double kp_delta(const Words& w, double inv_alpha, const m64::LogEntry* tab)
     {
-        const double cs = cospi(2.0 * uniform(w.w1));
-        return -(::log(uniform(w.w0)) + cs * cs * ::log(uniform(w.w2))) * inv_alpha;
+        const double c2 = m64::cos2_2pi_uniform(w.w1);
+        const double l0 = m64::log_uniform(uniform(w.w0), tab), l2 = m64::log_uniform(uniform(w.w2), tab);
+        return -fma(c2, l2, l0) * inv_alpha;
     }
     static __device__ __forceinline__ double kp_delta_refined(const Words&, double, double delta) { return delta; }
     static __device__ __forceinline__ double tiny() { return 1e-30; }

@@ -32,6 +32,10 @@ namespace su2 {
 // touched by any later sub-step of the sweep and each of their plaquettes holds exactly
 // one odd-parity mu-link, so the three kernels (1,1), (2,1), (3,1) together sum every
 // plaquette of the final configuration exactly once.
+// log table of su2_math64.cuh (fp64 kernels; 2 KB, stays in L1)
+__device__ const m64::LogEntry kLogTab[m64::kLogEntries] = {
+#include "su2_log_table.inc"
+};
 template <typename Real>
 struct Staple18 {  // the 18 links of one staple sum, per direction nu != mu (i = 0..2)
     Quat<Real> a[3], b[3], cc[3], a2[3], b2[3], c2[3];
@@ -75,7 +79,8 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
 // rows 3 (products) to 6: staple sum, Philox, Kennedy-Pendleton, compose, store
 template <typename Real, int MU, int P, bool MEAS>
 __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteIdx ix, uint32_t sweep, Real inv_beta,
-                                            const HbParams<Real>& hp, int* __restrict__ err)
+                                            const HbParams<Real>& hp, const m64::LogEntry* tab,
+                                            int* __restrict__ err)
 {
     const Quat<Real>*a = q.a, *b = q.b, *cc = q.cc, *a2 = q.a2, *b2 = q.b2, *c2 = q.c2;
     const int h = ix.h, r = ix.r;
@@ -120,7 +125,7 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
         uint32_t n = 1;
         for (;;) {
             const Words w = philox_keyed(s, sweep, tag, n, hp.rk);
-            delta = M<Real>::kp_delta(w, inv_alpha);
+            delta = M<Real>::kp_delta(w, inv_alpha, tab);
             const Real Rppp = M<Real>::uniform(w.w3);
             if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) {
                 delta = M<Real>::kp_delta_refined(w, inv_alpha, delta);
@@ -171,7 +176,7 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     run_state(hp, sweep, inv_beta);
     Staple18<Real> q;
     const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q);
-    return update_link<Real, MU, P, MEAS>(q, ix, sweep, inv_beta, hp, err);
+    return update_link<Real, MU, P, MEAS>(q, ix, sweep, inv_beta, hp, kLogTab, err);
 }
 
 // Resident CTAs per SM that ptxas must allow: this is the register budget that lets it
