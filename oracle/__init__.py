@@ -31,7 +31,7 @@ def lib():
             f = getattr(_lib, f"orc_uniform_{m}")
             f.argtypes = [C.c_uint32]
             f.restype = areal
-            for name in ("orc_init", "orc_staple", "orc_staple_norms", "orc_kp_x0", "orc_heatbath_link",
+            for name in ("orc_init", "orc_staple", "orc_staple_norms", "orc_kp_x0", "orc_creutz_x0", "orc_set_draw", "orc_heatbath_link",
                          "orc_heatbath_substep", "orc_heatbath_sweep", "orc_mean_plaquette",
                          "orc_plaquette_at", "orc_polyakov_loop", "orc_gauge_transform"):
                 getattr(_lib, f"{name}_{m}").restype = C.c_int
@@ -111,6 +111,25 @@ def kp_x0(alpha, seed, s, sweep, mode="f64"):
                                             C.byref(x0), C.byref(tr))
     _check(rc, "kp_x0")
     return x0.value, tr.value
+
+
+def creutz_x0(alpha, seed, s, sweep, mode="f64"):
+    x0 = C.c_double(0)
+    tr = C.c_int(0)
+    rc = getattr(lib(), f"orc_creutz_x0_{mode}")(C.c_double(alpha), C.c_uint64(seed), C.c_uint32(s),
+                                                C.c_uint32(sweep), C.byref(x0), C.byref(tr))
+    _check(rc, "creutz_x0")
+    return x0.value, tr.value
+
+
+DRAW = {"kp": 0, "auto": 1, "creutz": 2}
+ALPHA_C = 1.6847  # [R15]
+
+
+def set_draw(method, mode="f64"):
+    """Draw of x0 used by the heat-bath calls of `mode` from now on: 'kp' (default, [R6]),
+    'creutz' ([R15]) or 'auto' (per link: Creutz iff alpha < ALPHA_C). Process-wide per mode."""
+    _check(getattr(lib(), f"orc_set_draw_{mode}")(DRAW[method]), "set_draw")
 
 
 def heatbath_link(dims, links, beta, seed, sweep, s, mu, mode="f64"):

@@ -32,7 +32,8 @@
  * of plaquettes; KP law vs I2/I1 and the closed-form acceptance; single-link
  * heat bath on 2^4 vs brute-force quadrature; cold plaquette = 1; gauge
  * invariance; Polyakov centre flip; D=2 equilibrium plaquette = I2(b)/I1(b);
- * D=4 Schwinger–Dyson identity; visiting-order independence.
+ * D=4 Schwinger–Dyson identity; visiting-order independence; Creutz draw [R15]
+ * vs I2/I1, (pi/2) I1/sinh and the quadrature CDF.
  * Unpinned: D=4 <L> values across the N_t=4 transition (the paper prints none).
  */
 #include <math.h>
@@ -69,12 +70,14 @@ typedef ORC_AREAL AREAL; /* arithmetic type */
 #if defined(ORC_AREAL_IS_FLOAT)
 #define A_SQRT sqrtf
 #define A_LOG logf
+#define A_EXP expf
 #define A_COS cosf
 #define A_SIN sinf
 #define A_TWO_PI 6.28318530717958647692f
 #else
 #define A_SQRT sqrt
 #define A_LOG log
+#define A_EXP exp
 #define A_COS cos
 #define A_SIN sin
 #define A_TWO_PI 6.28318530717958647692
@@ -380,6 +383,66 @@ int FN(orc_kp_x0)(double alpha, uint64_t seed, uint32_t s, uint32_t sweep, doubl
 }
 
 /* ====================================================================== */
+/* Creutz's original draw [R15] (Creutz 1980; north_star "Creutz/Kennedy-     */
+/* Pendleton"): propose x0 with density ~ exp(alpha x0) on [-1,1] by          */
+/* inversion, accept with probability sqrt(1 - x0^2). Trial n = 1,2,...:      */
+/*   (R, R', ., .) = u(words of Philox(..., n))                               */
+/*   delta = 1 - x0 = -ln( R + (1 - R) exp(-2 alpha) ) / alpha                */
+/*   accept iff R'^2 <= 1 - x0^2 = delta (2 - delta).                         */
+/* Same target law as [R6]; acceptance (pi/2) I1(alpha)/sinh(alpha), which    */
+/* beats KP's below alpha_c = 1.6847 (where the two are equal).               */
+/* *margin = smallest |R'^2 - delta(2-delta)| over the trials made.           */
+/* ====================================================================== */
+#define ORC_DRAW_KP 0
+#define ORC_DRAW_AUTO 1   /* per link: Creutz iff alpha < ORC_ALPHA_C */
+#define ORC_DRAW_CREUTZ 2 /* always Creutz */
+#define ORC_ALPHA_C 1.6847
+static int g_draw_method = ORC_DRAW_KP;
+
+int FN(orc_set_draw)(int method)
+{
+    if (method < 0 || method > 2) return ORC_EARG;
+    g_draw_method = method;
+    return ORC_OK;
+}
+
+static int creutz_delta(AREAL alpha, uint64_t seed, uint32_t s, uint32_t sweep, uint32_t parity,
+                        uint32_t mu, AREAL *delta_out, int *trials_out, AREAL *margin_out)
+{
+    AREAL margin = (AREAL)1e30;
+    AREAL E = A_EXP(-(AREAL)2 * alpha);
+    for (int n = 1; n <= ORC_MAX_TRIALS; ++n) {
+        uint32_t w[4];
+        draw_words(seed, s, sweep, 0u, parity, mu, (uint32_t)n, w);
+        AREAL R = uniform_from_word(w[0]);
+        AREAL Rp = uniform_from_word(w[1]);
+        AREAL delta = -A_LOG(R + ((AREAL)1 - R) * E) / alpha;
+        AREAL lhs = Rp * Rp;
+        AREAL rhs = delta * ((AREAL)2 - delta);
+        AREAL m = lhs - rhs;
+        if (m < 0) m = -m;
+        if (m < margin) margin = m;
+        if (lhs <= rhs) {
+            *delta_out = delta;
+            if (trials_out) *trials_out = n;
+            if (margin_out) *margin_out = margin;
+            return ORC_OK;
+        }
+    }
+    return ORC_ETRIALS;
+}
+
+/* Stand-alone Creutz draw for the x0-law pins: returns x0 = 1 - delta. */
+int FN(orc_creutz_x0)(double alpha, uint64_t seed, uint32_t s, uint32_t sweep, double *x0_out, int *trials_out)
+{
+    AREAL delta;
+    int rc = creutz_delta((AREAL)alpha, seed, s, sweep, 0u, 0u, &delta, trials_out, NULL);
+    if (rc) return rc;
+    *x0_out = (double)((AREAL)1 - delta);
+    return ORC_OK;
+}
+
+/* ====================================================================== */
 /* Heat-bath update of one link [R2][R4][R6][R7][R8]. Local weight           */
 /* exp(beta 1/2 Tr(U v)) = exp(beta k 1/2 Tr(U Vbar)), k = |v|, Vbar = v/k.  */
 /* X = U Vbar has density ~ exp(alpha x0) dHaar, alpha = beta k; U' = X Vbar^dag. */
@@ -414,8 +477,17 @@ static int heatbath_link(const geom_t *g, const REAL *links, double beta, uint64
     AREAL alpha = (AREAL)beta * k;
 
     AREAL delta;
-    int rc = kp_delta(alpha, seed, (uint32_t)s, sweep, (uint32_t)p, (uint32_t)mu, &delta, trials, margin);
+    int rc;
+    if (g_draw_method == ORC_DRAW_CREUTZ || (g_draw_method == ORC_DRAW_AUTO && alpha < (AREAL)ORC_ALPHA_C))
+        rc = creutz_delta(alpha, seed, (uint32_t)s, sweep, (uint32_t)p, (uint32_t)mu, &delta, trials, margin); /* [R15] */
+    else
+        rc = kp_delta(alpha, seed, (uint32_t)s, sweep, (uint32_t)p, (uint32_t)mu, &delta, trials, margin);
     if (rc) return rc;
+    if (g_draw_method == ORC_DRAW_AUTO && margin) { /* a rounding-decided choice of method is excusable too */
+        AREAL mc = alpha - (AREAL)ORC_ALPHA_C;
+        if (mc < 0) mc = -mc;
+        if (mc < *margin) *margin = mc;
+    }
 
     /* [R7] direction uniform on the sphere of radius sqrt(1-x0^2) = sqrt(delta(2-delta)) */
     AREAL x0 = (AREAL)1 - delta;

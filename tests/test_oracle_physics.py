@@ -336,3 +336,94 @@ def test_degenerate_staple_gives_haar_element_independent_of_beta():
     # a neighbouring link with a non-zero staple is updated normally
     u4, tr4, _ = oracle.heatbath_link(dims, L, 2.3, 5, 0, s + 1, mu)
     assert tr4 >= 1
+
+
+# ---------------------------------------------------------------- Creutz draw [R15]
+@pytest.fixture
+def draw_mode():
+    """Switches the oracle's draw for one test and restores the default (KP) afterwards."""
+    def use(method, mode="f64"):
+        oracle.set_draw(method, mode)
+    yield use
+    for m in ("f64", "f32", "f32x"):
+        oracle.set_draw("kp", m)
+
+
+@pytest.mark.parametrize("alpha,mean_x0,acc", [(0.5, 0.123718, 0.777400), (1.0, 0.240194, 0.755402),
+                                               (2.0, 0.433127, 0.688906)])
+def test_creutz_draw_matches_closed_forms(alpha, mean_x0, acc):
+    """Same target law as KP: <x0> = I2/I1 (0.123718 and 0.240194 are SURVEY.md §8(c)'s strong-coupling
+    and D=2 values of that ratio); acceptance = (pi/2) I1(a)/sinh(a) (0.755 at
+    a = 1); CDF of sqrt(1-x^2) e^{a x} by quadrature (KS)."""
+    assert abs(RATIO(alpha) - mean_x0) < 2e-6
+    assert abs(np.pi / 2 * special.iv(1, alpha) / np.sinh(alpha) - acc) < 2e-6
+    n = 40000
+    x0 = np.empty(n)
+    trials = np.empty(n, dtype=np.int64)
+    for i in range(n):
+        x0[i], trials[i] = oracle.creutz_x0(alpha, 4321, i, 0)
+    dens = lambda x: np.sqrt(max(0.0, 1 - x * x)) * np.exp(alpha * (x - 1))
+    Z = integrate.quad(dens, -1, 1, epsabs=1e-13)[0]
+    var = integrate.quad(lambda x: x * x * dens(x), -1, 1, epsabs=1e-13)[0] / Z - RATIO(alpha) ** 2
+    assert abs(x0.mean() - RATIO(alpha)) < 4.5 * np.sqrt(var / n)
+    p_acc = 1.0 / trials.mean()
+    assert abs(p_acc - acc) < 4.5 * np.sqrt(acc * (1 - acc) / n) / acc
+    grid = np.linspace(-1, 1, 4001)
+    pdf = np.sqrt(np.clip(1 - grid**2, 0, None)) * np.exp(alpha * (grid - 1))
+    cdfg = integrate.cumulative_trapezoid(pdf, grid, initial=0)
+    cdfg /= cdfg[-1]
+    assert stats.kstest(x0, lambda x: np.interp(x, grid, cdfg)).pvalue > 1e-4
+    assert (x0 >= -1).all() and (x0 < 1).all()
+
+
+def test_acceptance_crossover_is_alpha_c():
+    """[R15]: ALPHA_C is where KP's acceptance sqrt(2 pi a) e^-a I1(a) equals Creutz's (pi/2) I1(a)/sinh(a)."""
+    a = oracle.ALPHA_C
+    kp = np.sqrt(2 * np.pi * a) * special.ive(1, a)
+    cr = np.pi / 2 * special.iv(1, a) / np.sinh(a)
+    assert abs(kp - cr) < 2e-5
+    assert np.sqrt(2 * np.pi * 1.0) * special.ive(1, 1.0) < np.pi / 2 * special.iv(1, 1.0) / np.sinh(1.0)
+    assert np.sqrt(2 * np.pi * 3.0) * special.ive(1, 3.0) > np.pi / 2 * special.iv(1, 3.0) / np.sinh(3.0)
+
+
+def test_auto_draw_selects_per_link_and_samples_the_boltzmann_weight(draw_mode):
+    """'auto' = Creutz iff alpha < ALPHA_C, per link. On a 2^4 hot lattice at beta = 0.5 some links
+    have alpha below and some above: the new link equals the always-Creutz result on the former
+    and the KP result on the latter; and the single-link mean is (I2/I1)(beta k) Vbar^dagger."""
+    dims, beta, seed = [2, 2, 2, 2], 0.5, 23
+    L = oracle.init(dims, "hot", seed)
+    alpha = beta * oracle.staple_norms(dims, L)
+    assert (alpha < oracle.ALPHA_C).any() and (alpha > oracle.ALPHA_C).any()
+    res = {}
+    for method in ("kp", "creutz", "auto"):
+        draw_mode(method)
+        res[method] = np.array([[oracle.heatbath_link(dims, L, beta, seed, 0, s, mu)[0] for mu in range(4)]
+                                for s in range(16)])
+    low = alpha < oracle.ALPHA_C
+    assert (res["auto"][low] == res["creutz"][low]).all()
+    assert (res["auto"][~low] == res["kp"][~low]).all()
+    assert not (res["kp"][low] == res["creutz"][low]).all()
+    # law of the updated link under 'auto' at a link with small alpha
+    s, mu = np.argwhere(low)[0]
+    v = oracle.staple(dims, L, int(s), int(mu))
+    k = np.linalg.norm(v)
+    n = 30000
+    U = np.array([oracle.heatbath_link(dims, L, beta, seed, i, int(s), int(mu))[0] for i in range(n)])
+    assert np.abs((U**2).sum(1) - 1).max() < 9e-16
+    want = RATIO(beta * k) * v * [1, -1, -1, -1] / k
+    assert np.abs(U.mean(0) - want).max() < 4.5 * 0.5 / np.sqrt(n)
+
+
+def test_d2_equilibrium_plaquette_with_creutz_draw(draw_mode):
+    """Whole chain with the always-Creutz draw, D = 2: <1/2 Tr P> = I2(beta)/I1(beta) = 0.240194 at beta = 1."""
+    draw_mode("creutz")
+    dims, beta = [8, 8], 1.0
+    L = oracle.init(dims, "hot", 3)
+    vals = []
+    for sw in range(1200):
+        oracle.heatbath_sweep(dims, L, beta, 3, sw)
+        if sw >= 100:
+            vals.append(oracle.mean_plaquette(dims, L))
+    vals = np.array(vals)
+    b = vals[: len(vals) // 20 * 20].reshape(20, -1).mean(1)
+    assert abs(vals.mean() - 0.240194) < 4.5 * b.std(ddof=1) / np.sqrt(20)
