@@ -100,6 +100,24 @@ SU2_API int su2_set_seed(su2_lattice* lat, uint64_t seed);
  * Errors: SU2_EARG (beta <= 0 or not finite), SU2_ESTATE, SU2_ECUDA. */
 SU2_API int su2_heatbath_sweep(su2_lattice* lat, double beta, uint32_t sweep_idx);
 
+/* S8(f) NEXT-3(i), north_star "Creutz/Kennedy-Pendleton" [R15]: which draw of x0 (density
+ * ~ sqrt(1-x0^2) exp(alpha x0), alpha = beta k) later sweeps of this handle use.
+ *   SU2_DRAW_KP     Kennedy-Pendleton on every link [R6] (the default; alpha >= 5 on every
+ *                   BASELINE config, acceptance 0.93-0.99)
+ *   SU2_DRAW_CREUTZ Creutz's original draw on every link: trial n = 1,2,...: (R, R', ., .) =
+ *                   u(words of Philox(..., n)); delta = -ln(R + (1-R) exp(-2 alpha))/alpha;
+ *                   accept iff R'^2 <= delta (2 - delta); x0 = 1 - delta. Acceptance
+ *                   (pi/2) I1(alpha)/sinh(alpha): 0.76 at alpha = 1, 0.22 at alpha = 32.
+ *   SU2_DRAW_AUTO   per link: Creutz iff alpha < SU2_ALPHA_C (where the two acceptances
+ *                   are equal), else KP. For strong coupling (beta <~ 0.5).
+ * Direction, composition [R7] and the Philox keying [R5] are the same for both.
+ * Errors: SU2_EARG. */
+#define SU2_DRAW_KP 0
+#define SU2_DRAW_AUTO 1
+#define SU2_DRAW_CREUTZ 2
+#define SU2_ALPHA_C 1.6847
+SU2_API int su2_set_draw(su2_lattice* lat, int method);
+
 /* One sub-step (mu, parity) only — the unit the tests compare against the oracle. */
 SU2_API int su2_heatbath_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, int mu, int parity);
 

@@ -30,6 +30,7 @@ struct su2_lattice {
     cudaEvent_t run_ev_in, run_ev_out;
     cudaGraphExec_t run_exec;
     bool run_graphs;   // SU2HB_NO_GRAPH=1 disables (A/B timing only)
+    double creutz_below;  // [R15] su2_set_draw: 0 (KP), SU2_ALPHA_C (auto) or +inf (Creutz)
     void* stage;       // canonical-order staging buffer of su2_get_links / su2_set_links (lazy, kept)
     int sticky;  // sticky error code
     char msg[256];
@@ -68,8 +69,9 @@ static void enqueue_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, i
     const int idx = 2 * mu + parity;
     const bool overlap = allow_overlap && lat->pdl && lat->last_substep == (idx + 7) % 8;
     if (!state) st = lat->stream;
-    lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, parity, beta, lat->seed,
-                                             sweep_idx, lat->sc.err, epart, state, overlap, st);
+    lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, parity, beta,
+                                             lat->creutz_below, lat->seed, sweep_idx, lat->sc.err, epart, state,
+                                             overlap, st);
     lat->last_substep = idx;
 }
 
@@ -202,6 +204,26 @@ extern "C" int su2_set_seed(su2_lattice* lat, uint64_t seed)
 {
     ENTER(lat);
     lat->seed = seed;
+    return SU2_OK;
+}
+
+extern "C" int su2_set_draw(su2_lattice* lat, int method)
+{
+    ENTER(lat);
+    NOT_A_SUBSTEP(lat);
+    double cb;
+    switch (method) {
+        case SU2_DRAW_KP: cb = 0.0; break;
+        case SU2_DRAW_AUTO: cb = SU2_ALPHA_C; break;
+        case SU2_DRAW_CREUTZ: cb = INFINITY; break;
+        default: return fail(lat, SU2_EARG, "su2_set_draw: bad method");
+    }
+    if (cb != lat->creutz_below && lat->run_exec) {  // the captured step holds the other kernels
+        CK(lat, cudaStreamSynchronize(lat->run_stream));
+        cudaGraphExecDestroy(lat->run_exec);
+        lat->run_exec = nullptr;
+    }
+    lat->creutz_below = cb;
     return SU2_OK;
 }
 

@@ -257,6 +257,7 @@ struct M<float> {
     static __device__ __forceinline__ float one_two(uint32_t w) { return __uint_as_float(0x3F800000u | (w >> 9)); }
     static __device__ __forceinline__ float uniform(uint32_t w) { return one_two(w) - 0.99999994f; }
     static __device__ __forceinline__ float log(float x) { return logf(x); }
+    static __device__ __forceinline__ float exp(float x) { return expf(x); }
     static __device__ __forceinline__ float sqrt(float x) { return sqrtf(x); }
     static __device__ __forceinline__ float rcp(float x) { return 1.0f / x; }
     // MUFU approximations (<= 2 ulp): the fp32 link tolerance is 1e-5
@@ -322,6 +323,7 @@ struct M<double> {
         return fma((double)w, 1.0 / 4294967296.0, 1.0 / 8589934592.0);
     }
     static __device__ __forceinline__ double log(double x) { return ::log(x); }
+    static __device__ __forceinline__ double exp(double x) { return ::exp(x); }
     static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
     static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
     // su2_math64.cuh: functions specialised to the arguments of this path
@@ -379,6 +381,7 @@ struct __align__(16) HbParams {
     const RunState* state;                        // non-null inside su2_run: sweep and 1/beta come from here
     Real inv_beta;
     uint32_t sweep;
+    Real creutz_below;  // [R15] ALT kernels: Creutz's draw where alpha < this (0 = never, +inf = always)
 };
 
 // [R9] Shoemake: uniform unit quaternion from three uniforms

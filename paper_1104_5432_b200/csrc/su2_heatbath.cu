@@ -77,7 +77,7 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
 }
 
 // rows 3 (products) to 6: staple sum, Philox, Kennedy-Pendleton, compose, store
-template <typename Real, int MU, int P, bool MEAS>
+template <typename Real, int MU, int P, bool MEAS, bool ALT>
 __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteIdx ix, uint32_t sweep, Real inv_beta,
                                             const HbParams<Real>& hp, const m64::LogEntry* tab,
                                             int* __restrict__ err)
@@ -120,21 +120,38 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
     } else {
         const Real rk = M<Real>::rsqrt(k2);       // 1/k
         const Real inv_alpha = rk * inv_beta;  // 1/(beta k)
-        // [R6] Kennedy-Pendleton
         Real delta = 0;
         uint32_t n = 1;
-        for (;;) {
-            const Words w = philox_keyed(s, sweep, tag, n, hp.rk);
-            delta = M<Real>::kp_delta(w, inv_alpha, tab);
-            const Real Rppp = M<Real>::uniform(w.w3);
-            if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) {
-                delta = M<Real>::kp_delta_refined(w, inv_alpha, delta);
-                break;
+        if (ALT && inv_alpha * hp.creutz_below > (Real)1) {
+            // [R15] Creutz: propose x0 ~ exp(alpha x0) by inversion, accept with sqrt(1 - x0^2).
+            // The rare small-alpha path: accurate library exp/log in both precisions.
+            const Real E = M<Real>::exp((Real)-2 / inv_alpha);
+            for (;;) {
+                const Words w = philox_keyed(s, sweep, tag, n, hp.rk);
+                const Real R = M<Real>::uniform(w.w0), Rp = M<Real>::uniform(w.w1);
+                delta = -M<Real>::log(R + ((Real)1 - R) * E) * inv_alpha;
+                if (Rp * Rp <= delta * ((Real)2 - delta)) break;
+                if (++n > 10000u) {
+                    atomicOr(err, 1);
+                    delta = 0;
+                    break;
+                }
             }
-            if (++n > 10000u) {  // unreachable for alpha >~ 1e-4; flag, keep x0 = 1
-                atomicOr(err, 1);
-                delta = 0;
-                break;
+        } else {
+            // [R6] Kennedy-Pendleton
+            for (;;) {
+                const Words w = philox_keyed(s, sweep, tag, n, hp.rk);
+                delta = M<Real>::kp_delta(w, inv_alpha, tab);
+                const Real Rppp = M<Real>::uniform(w.w3);
+                if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) {
+                    delta = M<Real>::kp_delta_refined(w, inv_alpha, delta);
+                    break;
+                }
+                if (++n > 10000u) {  // unreachable for alpha >~ 1e-4; flag, keep x0 = 1
+                    atomicOr(err, 1);
+                    delta = 0;
+                    break;
+                }
             }
         }
         // [R7] direction on the sphere of radius sqrt(delta(2-delta)), compose with Vbar^dagger
@@ -165,7 +182,7 @@ __device__ __forceinline__ void run_state(const HbParams<Real>& hp, uint32_t& sw
     }
 }
 
-template <typename Real, int MU, int P, bool MEAS>
+template <typename Real, int MU, int P, bool MEAS, bool ALT>
 __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
                                               int* __restrict__ err)
 {
@@ -176,7 +193,7 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     run_state(hp, sweep, inv_beta);
     Staple18<Real> q;
     const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q);
-    return update_link<Real, MU, P, MEAS>(q, ix, sweep, inv_beta, hp, kLogTab, err);
+    return update_link<Real, MU, P, MEAS, ALT>(q, ix, sweep, inv_beta, hp, kLogTab, err);
 }
 
 // Resident CTAs per SM that ptxas must allow: this is the register budget that lets it
@@ -198,12 +215,12 @@ struct MinBlocks<double> {
 
 // tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile;
 // grid = (nb0, nb1, nb2*nb3): x fastest, so CTAs are scheduled roughly in memory order.
-template <typename Real, int MU, int P, bool MEAS, int LHX, int LY, int LZ, int LT>
+template <typename Real, int MU, int P, bool MEAS, bool ALT, int LHX, int LY, int LZ, int LT>
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::value)
     heatbath_tiled_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
     const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z);
-    const Real e = heatbath_site<Real, MU, P, MEAS>(g, c, hp, err);
+    const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, err);
     if (MEAS) {  // one fp64 partial per CTA, fixed order
         __shared__ double red[kBlock / 32];
         const double tot = block_sum_end(e, red);
@@ -212,7 +229,7 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::va
 }
 
 // linear launch: thread i <-> half-index h = i; any even extents
-template <typename Real, int MU, int P, bool MEAS>
+template <typename Real, int MU, int P, bool MEAS, bool ALT>
 __global__ void __launch_bounds__(kBlock)
     heatbath_linear_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
@@ -226,7 +243,7 @@ __global__ void __launch_bounds__(kBlock)
         c.y = (int)(q - q2 * (uint32_t)g.n[1]);
         c.t = (int)(q2 / (uint32_t)g.n[2]);
         c.z = (int)(q2 - (uint32_t)c.t * (uint32_t)g.n[2]);
-        e = heatbath_site<Real, MU, P, MEAS>(g, c, hp, err);
+        e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, err);
     }
     if (MEAS) {
         __shared__ double red[kBlock / 32];
@@ -301,14 +318,16 @@ static void launch_ex(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStrea
     cudaLaunchKernelEx(&cfg, kernel, args...);
 }
 
-template <typename Real, int MU, int P, bool MEAS>
-static int launch_substep_t(void* links, const Geom& g, double beta, uint64_t seed, uint32_t sweep, int* err,
-                            double* epart, const RunState* state, bool overlap, cudaStream_t st)
+template <typename Real, int MU, int P, bool MEAS, bool ALT>
+static int launch_substep_t(void* links, const Geom& g, double beta, double creutz_below, uint64_t seed,
+                            uint32_t sweep, int* err, double* epart, const RunState* state, bool overlap,
+                            cudaStream_t st)
 {
     typedef typename LinkPtr<Real>::type L;
     HbParams<Real> hp;
     hp.inv_beta = (Real)(1.0 / beta);
     hp.sweep = sweep;
+    hp.creutz_below = (Real)creutz_below;
     hp.rk = expand_keys(seed);
     for (int nu = 0; nu < 4; ++nu) {
         hp.same[nu] = (const L*)links + (size_t)(P * 4 + nu) * g.vh;
@@ -319,15 +338,15 @@ static int launch_substep_t(void* links, const Geom& g, double beta, uint64_t se
     hp.state = state;
     const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
     if (g.tile == 0) {
-        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>,
+        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>,
                   grid, dim3(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3])), st, overlap, g, hp,
                   err);
     } else if (g.tile == 1) {
-        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3]>,
+        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3]>,
                   grid, dim3(1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3])), st, overlap, g, hp,
                   err);
     } else {
-        launch_ex(heatbath_linear_kernel<Real, MU, P, MEAS>, dim3((unsigned)heatbath_ctas(g)), dim3(kBlock), st,
+        launch_ex(heatbath_linear_kernel<Real, MU, P, MEAS, ALT>, dim3((unsigned)heatbath_ctas(g)), dim3(kBlock), st,
                   overlap, g, hp, err);
     }
     return 1;
@@ -340,41 +359,49 @@ size_t heatbath_ctas(const Geom& g)
     return ((size_t)g.vh + kBlock - 1) / kBlock;
 }
 
-template <typename Real>
-static int launch_substep_p(void* links, const Geom& g, int mu, int parity, double beta, uint64_t seed,
+template <typename Real, bool ALT>
+static int launch_substep_p(void* links, const Geom& g, int mu, int parity, double beta, double cb, uint64_t seed,
                             uint32_t sweep, int* err, double* epart, const RunState* state, bool overlap,
                             cudaStream_t st)
 {
+#define SU2_HB(MU_, P_, MEAS_, EP_) \
+    return launch_substep_t<Real, MU_, P_, MEAS_, ALT>(links, g, beta, cb, seed, sweep, err, EP_, state, overlap, st)
     if (epart && parity == 1 && mu >= 1) {  // the three measuring kernels
         switch (mu) {
-            case 1: return launch_substep_t<Real, 1, 1, true>(links, g, beta, seed, sweep, err, epart, state, overlap, st);
-            case 2: return launch_substep_t<Real, 2, 1, true>(links, g, beta, seed, sweep, err, epart, state, overlap, st);
-            default: return launch_substep_t<Real, 3, 1, true>(links, g, beta, seed, sweep, err, epart, state, overlap, st);
+            case 1: SU2_HB(1, 1, true, epart);
+            case 2: SU2_HB(2, 1, true, epart);
+            default: SU2_HB(3, 1, true, epart);
         }
     }
     switch (mu * 2 + parity) {
-        case 0: return launch_substep_t<Real, 0, 0, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
-        case 1: return launch_substep_t<Real, 0, 1, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
-        case 2: return launch_substep_t<Real, 1, 0, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
-        case 3: return launch_substep_t<Real, 1, 1, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
-        case 4: return launch_substep_t<Real, 2, 0, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
-        case 5: return launch_substep_t<Real, 2, 1, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
-        case 6: return launch_substep_t<Real, 3, 0, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
-        default: return launch_substep_t<Real, 3, 1, false>(links, g, beta, seed, sweep, err, nullptr, state, overlap, st);
+        case 0: SU2_HB(0, 0, false, nullptr);
+        case 1: SU2_HB(0, 1, false, nullptr);
+        case 2: SU2_HB(1, 0, false, nullptr);
+        case 3: SU2_HB(1, 1, false, nullptr);
+        case 4: SU2_HB(2, 0, false, nullptr);
+        case 5: SU2_HB(2, 1, false, nullptr);
+        case 6: SU2_HB(3, 0, false, nullptr);
+        default: SU2_HB(3, 1, false, nullptr);
     }
+#undef SU2_HB
 }
 
 // `overlap` may be true only if the launch before this one on `st` was the canonical
 // predecessor sub-step [R4] of the same lattice (see heatbath_site). `epart` (nullable):
 // where the sub-steps (mu >= 1, parity 1) store their heatbath_ctas(g) fused-plaquette
 // partials; ignored by the other sub-steps.
+// `creutz_below` [R15]: 0 = Kennedy-Pendleton everywhere (the hot-path kernels); otherwise the ALT
+// kernels, which use Creutz's draw on links with alpha < creutz_below (+inf = on every link).
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
-                            uint64_t seed, uint32_t sweep, int* err, double* epart, const RunState* state,
-                            bool overlap, cudaStream_t st)
+                            double creutz_below, uint64_t seed, uint32_t sweep, int* err, double* epart,
+                            const RunState* state, bool overlap, cudaStream_t st)
 {
-    return precision == 32
-               ? launch_substep_p<float>(links, g, mu, parity, beta, seed, sweep, err, epart, state, overlap, st)
-               : launch_substep_p<double>(links, g, mu, parity, beta, seed, sweep, err, epart, state, overlap, st);
+    const bool alt = creutz_below > 0.0;
+#define SU2_HB(REAL_, ALT_) \
+    launch_substep_p<REAL_, ALT_>(links, g, mu, parity, beta, creutz_below, seed, sweep, err, epart, state, overlap, st)
+    if (precision == 32) return alt ? SU2_HB(float, true) : SU2_HB(float, false);
+    return alt ? SU2_HB(double, true) : SU2_HB(double, false);
+#undef SU2_HB
 }
 
 int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st)

@@ -41,8 +41,8 @@ size_t partials_needed(const Geom& g);
 // each returns the number of kernels it enqueued (0 on launch failure; check cudaGetLastError)
 int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st);
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
-                            uint64_t seed, uint32_t sweep, int* err, double* epart, const RunState* state, bool overlap,
-                            cudaStream_t st);
+                            double creutz_below, uint64_t seed, uint32_t sweep, int* err, double* epart,
+                            const RunState* state, bool overlap, cudaStream_t st);
 size_t heatbath_ctas(const Geom& g);
 int launch_final_sum(const double* partials, size_t n, double scale, double* dev_dst, cudaStream_t st);
 // su2_run: the destination is state->out[2*state->index + slot]; `advance` also bumps sweep and index

@@ -423,3 +423,84 @@ def test_run_equals_step_by_step_calls_bitwise(pkg, dims, prec, graphs, monkeypa
         assert_links_match(b.get_links(), L, 64)
     a.close()
     b.close()
+
+
+# ---------------------------------------------------------------- Creutz draw [R15] (S8(f) NEXT-3(i))
+@pytest.fixture
+def oracle_draw():
+    def use(method):
+        for m in ("f64", "f32", "f32x"):
+            oracle.set_draw(method, m)
+    yield use
+    for m in ("f64", "f32", "f32x"):
+        oracle.set_draw("kp", m)
+
+
+@pytest.mark.parametrize("method,beta", [("creutz", 0.3), ("creutz", 2.3), ("auto", 0.3), ("auto", 0.7), ("auto", 2.3)])
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", [(16, 8, 8, 4), (32, 4, 4, 2), (8, 8, 8, 8), (6, 4, 10, 2)])
+def test_creutz_and_auto_draw_match_oracle_teacher_forced(pkg, oracle_draw, dims, prec, method, beta):
+    """Sub-steps with su2_set_draw(CREUTZ | AUTO) against the oracle in the same mode. At beta = 0.7
+    on a hot lattice alpha = beta k straddles ALPHA_C, so 'auto' takes both branches in one launch
+    (a choice decided by rounding, |alpha - ALPHA_C| tiny, is excused like a flipped accept)."""
+    mode = MODE[prec]
+    oracle_draw(method)
+    L = workloads.random_links(dims, 21, oracle.dtype(mode))
+    if method == "auto" and beta == 0.7:
+        a = beta * oracle.staple_norms(dims, L, mode)
+        assert (a < oracle.ALPHA_C).mean() > 0.2 and (a > oracle.ALPHA_C).mean() > 0.2
+    lat = pkg.Lattice(dims, prec)
+    lat.set_seed(33)
+    lat.set_draw(method)
+    V = oracle.volume(dims)
+    for mu, p in ((0, 0), (1, 1), (2, 0), (3, 1)):
+        lat.set_links(L)
+        lat.substep(beta, 4, mu, p)
+        g = lat.get_links()
+        mg, tr = np.ones((V, 4)), np.zeros((V, 4), np.int32)
+        oracle.heatbath_substep(dims, L, beta, 33, 4, mu, p, mode, margin=mg, trials=tr)
+        assert_links_match(g, L, prec, mg, max_flips=2, what=f"{method} mu={mu} p={p}")
+    lat.close()
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_auto_draw_equals_kp_bitwise_at_large_alpha(pkg, prec):
+    """beta = 6 on a smooth lattice: alpha ~ 30 everywhere, so AUTO must reproduce the KP sweep bit for bit
+    (the ALT kernels differ from the hot-path kernels only by the branch)."""
+    dims = (16, 8, 8, 4)
+    L = workloads.smooth_links(dims, 3, 0.05, np.float64 if prec == 64 else np.float32)
+    out = []
+    for method in ("kp", "auto"):
+        lat = pkg.Lattice(dims, prec)
+        lat.set_links(L)
+        lat.set_seed(8)
+        lat.set_draw(method)
+        for sw in range(3):
+            lat.sweep(6.0, sw)
+        out.append(lat.get_links())
+        lat.close()
+    assert (out[0] == out[1]).all()
+
+
+def test_run_follows_set_draw_and_bad_method_is_rejected(pkg):
+    """su2_run's captured step is rebuilt when the draw changes; results equal the step-by-step calls."""
+    import torch
+    dims, prec, beta, n = (16, 8, 8, 4), 64, 0.5, 4
+    a, b = pkg.Lattice(dims, prec), pkg.Lattice(dims, prec)
+    for lat in (a, b):
+        lat.init("hot", 6)
+    oa = torch.zeros(2 * n, dtype=torch.float64, device="cuda")
+    ob = torch.zeros(2 * n, dtype=torch.float64, device="cuda")
+    a.run(beta, 0, 2, oa)                      # captures the KP step
+    a.set_draw("auto")
+    a.run(beta, 2, 2, oa[4:])
+    for i in range(n):
+        if i == 2:
+            b.set_draw("auto")
+        b.sweep_measure(beta, i, ob, i)
+    torch.cuda.synchronize()
+    assert (a.get_links() == b.get_links()).all()
+    assert torch.equal(oa, ob)
+    with pytest.raises(pkg.SU2Error):
+        pkg.su2_set_draw(a.h, 7)
+    a.close(); b.close()
