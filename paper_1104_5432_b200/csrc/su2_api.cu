@@ -57,6 +57,9 @@ static int fail(su2_lattice* lat, int code, const char* what, cudaError_t ce = c
         if (!(lat)) return SU2_EARG;     \
         if ((lat)->sticky) return (lat)->sticky; \
     } while (0)
+// last_substep value after the Polyakov kernel of a step: sub-step (0,0) may overlap its tail
+// (it waits for it like for a predecessor sub-step; that kernel itself waited for (3,1))
+static const int kAfterStepTail = 8;
 // every entry point that enqueues anything other than a heat-bath sub-step
 #define NOT_A_SUBSTEP(lat) ((lat)->last_substep = -1)
 
@@ -67,7 +70,8 @@ static void enqueue_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, i
                             bool allow_overlap = true)
 {
     const int idx = 2 * mu + parity;
-    const bool overlap = allow_overlap && lat->pdl && lat->last_substep == (idx + 7) % 8;
+    const bool overlap = allow_overlap && lat->pdl &&
+                         (lat->last_substep == (idx + 7) % 8 || (idx == 0 && lat->last_substep == kAfterStepTail));
     if (!state) st = lat->stream;
     lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, parity, beta,
                                              lat->creutz_below, lat->seed, sweep_idx, lat->sc.err, epart, state,
@@ -138,6 +142,9 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.field, v3 * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.out, (2 + kMaxR) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.state, sizeof(RunState));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.slots, 2 * (v3 / 64 + 1) * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.ticket, sizeof(unsigned));
+    if (ce == cudaSuccess) ce = cudaMemset(lat->sc.ticket, 0, sizeof(unsigned));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.err, sizeof(int));
     if (ce == cudaSuccess) ce = cudaMemset(lat->sc.err, 0, sizeof(int));
     if (ce != cudaSuccess) {
@@ -172,6 +179,8 @@ extern "C" int su2_lattice_destroy(su2_lattice* lat)
     if (lat->stage) cudaFree(lat->stage);
     if (lat->sc.err) cudaFree(lat->sc.err);
     if (lat->sc.state) cudaFree(lat->sc.state);
+    if (lat->sc.slots) cudaFree(lat->sc.slots);
+    if (lat->sc.ticket) cudaFree(lat->sc.ticket);
     if (lat->run_exec) cudaGraphExecDestroy(lat->run_exec);
     if (lat->run_ev_in) cudaEventDestroy(lat->run_ev_in);
     if (lat->run_ev_out) cudaEventDestroy(lat->run_ev_out);
@@ -265,14 +274,14 @@ extern "C" int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_
     for (int mu = 0; mu < 4; ++mu)
         for (int p = 0; p < 2; ++p)
             enqueue_substep(lat, beta, sweep_idx, mu, p, (p == 1 && mu >= 1) ? lat->sc.epart + (mu - 1) * ctas : nullptr);
-    NOT_A_SUBSTEP(lat);
     if (event_after_sweep) CK(lat, cudaEventRecord((cudaEvent_t)event_after_sweep, lat->stream));
-    // the three partial sets cover every plaquette of the new configuration once
-    size_t np = 0;
-    lat->launches += launch_polyakov_partials(lat->links, lat->g, lat->precision, lat->sc, &np, lat->stream);
-    const double v3 = (double)lat->g.n[0] * lat->g.n[1] * lat->g.n[2];
-    lat->launches += launch_final_sum2(lat->sc.epart, 3 * ctas, 1.0 / (6.0 * 2.0 * (double)lat->g.vh),
-                                       lat->sc.partials, np, 1.0 / v3, dev_out + 2 * index, nullptr, lat->stream);
+    // the three partial sets cover every plaquette of the new configuration once;
+    // the Polyakov kernel also finishes both sums and, like a sub-step, may be
+    // scheduled while its predecessor (3,1) drains; the next sweep's (0,0) may follow it the same way
+    lat->launches += launch_polyakov_step(lat->links, lat->g, lat->precision, lat->sc, lat->sc.epart, 3 * ctas,
+                                          1.0 / (6.0 * 2.0 * (double)lat->g.vh), dev_out + 2 * index, nullptr,
+                                          lat->pdl && !event_after_sweep, lat->stream);
+    lat->last_substep = kAfterStepTail;
     CK(lat, cudaGetLastError());
     return SU2_OK;
 }
@@ -286,12 +295,10 @@ static void enqueue_run_step(su2_lattice* lat, cudaStream_t st, bool allow_overl
         for (int p = 0; p < 2; ++p)
             enqueue_substep(lat, 1.0, 0u, mu, p, (p == 1 && mu >= 1) ? lat->sc.epart + (mu - 1) * ctas : nullptr,
                             lat->sc.state, st, allow_overlap);
+    lat->launches += launch_polyakov_step(lat->links, lat->g, lat->precision, lat->sc, lat->sc.epart, 3 * ctas,
+                                          1.0 / (6.0 * 2.0 * (double)lat->g.vh), nullptr, lat->sc.state,
+                                          allow_overlap && lat->pdl, st);
     lat->last_substep = -1;
-    size_t np = 0;
-    lat->launches += launch_polyakov_partials(lat->links, lat->g, lat->precision, lat->sc, &np, st);
-    const double v3 = (double)lat->g.n[0] * lat->g.n[1] * lat->g.n[2];
-    lat->launches += launch_final_sum2(lat->sc.epart, 3 * ctas, 1.0 / (6.0 * 2.0 * (double)lat->g.vh),
-                                       lat->sc.partials, np, 1.0 / v3, nullptr, lat->sc.state, st);
 }
 
 // capture one step into an executable graph; with programmatic edges first, without if the
@@ -333,7 +340,7 @@ extern "C" int su2_run(su2_lattice* lat, double beta, uint32_t sweep_idx0, uint3
     CK(lat, cudaStreamWaitEvent(lat->run_stream, lat->run_ev_in, 0));
     lat->launches += launch_set_run_state(lat->sc.state, 1.0 / beta, dev_out, sweep_idx0, 0u, lat->run_stream);
     const bool graphs = lat->run_graphs && (lat->run_exec || build_run_graph(lat));
-    const uint64_t per_step = 8 + 2;
+    const uint64_t per_step = 8 + 1;
     for (uint32_t i = 0; i < n_steps; ++i) {
         if (graphs) {
             CK(lat, cudaGraphLaunch(lat->run_exec, lat->run_stream));

@@ -300,24 +300,6 @@ void choose_tiling(Geom& g)
     }
 }
 
-// One launch through cudaLaunchKernelEx; `overlap` adds the programmatic-stream-
-// serialization attribute (the kernel may start while its predecessor drains).
-template <typename... KArgs, typename... Args>
-static void launch_ex(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, bool overlap, Args... args)
-{
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = grid;
-    cfg.blockDim = block;
-    cfg.dynamicSmemBytes = 0;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = overlap ? 1 : 0;
-    cudaLaunchKernelEx(&cfg, kernel, args...);
-}
-
 template <typename Real, int MU, int P, bool MEAS, bool ALT>
 static int launch_substep_t(void* links, const Geom& g, double beta, double creutz_below, uint64_t seed,
                             uint32_t sweep, int* err, double* epart, const RunState* state, bool overlap,

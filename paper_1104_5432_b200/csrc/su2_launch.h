@@ -23,6 +23,24 @@ constexpr int kTiles[kNumTiles][4] = {{HB_T0, HB_T1, HB_T2, HB_T3},  // 16 x 4 x
 constexpr int kBlock = 256;                 // block size of every other kernel; part of the
                                             // definition of the fixed-order reductions
 
+// One launch through cudaLaunchKernelEx; `overlap` adds the programmatic-stream-
+// serialization attribute (the kernel may start while its predecessor drains).
+template <typename... KArgs, typename... Args>
+inline void launch_ex(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, bool overlap, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = overlap ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 struct Scratch {
     double* partials;   // [device] block partial sums (plaquette | polyakov | correlator)
     size_t n_partials;  // capacity in doubles
@@ -31,6 +49,8 @@ struct Scratch {
     double* out;        // [device] 2 + kMaxR doubles: plaquette, polyakov, correlator
     int* err;           // [device] sticky error flags (bit 0: KP trial cap hit)
     RunState* state;    // [device] loop state of su2_run
+    double* slots;      // [device] step tail: 2 doubles per CTA of the Polyakov kernel (<= V/Nt/64 + 1 CTAs)
+    unsigned* ticket;   // [device] step tail: arrival counter, zero between steps
 };
 constexpr int kMaxR = 128;
 
@@ -45,16 +65,14 @@ int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, i
                             const RunState* state, bool overlap, cudaStream_t st);
 size_t heatbath_ctas(const Geom& g);
 int launch_final_sum(const double* partials, size_t n, double scale, double* dev_dst, cudaStream_t st);
-// su2_run: the destination is state->out[2*state->index + slot]; `advance` also bumps sweep and index
-int launch_final_sum_state(const double* partials, size_t n, double scale, RunState* state, int slot, bool advance,
-                           cudaStream_t st);
-int launch_final_sum2(const double* pa, size_t na, double sa, const double* pb, size_t nb, double sb, double* dst,
-                      RunState* state, cudaStream_t st);
 int launch_set_run_state(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index,
                          cudaStream_t st);
-// Polyakov partials only (no final sum): used by su2_run, which sums them with launch_final_sum_state
+// Polyakov partials only (no final sum)
 int launch_polyakov_partials(const void* links, const Geom& g, int precision, const Scratch& sc, size_t* n_partials,
                              cudaStream_t st);
+int launch_polyakov_step(const void* links, const Geom& g, int precision, const Scratch& sc, const double* epart,
+                         size_t n_epart, double scale_plaq, double* dev_dst, RunState* state, bool overlap,
+                         cudaStream_t st);
 int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
                      cudaStream_t st);
 int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,

@@ -122,17 +122,73 @@ __global__ void __launch_bounds__(1024) final_sum_kernel(const double* __restric
     if (threadIdx.x == 0) dst[0] = tot * scale;
 }
 
+// ------------------------------------------------------------------ tail of a step
+// su2_heatbath_sweep_measure / su2_run: the Polyakov kernel is the last kernel of a step and
+// also finishes both observables (no separate final-sum launch). CTA b sums slice b of the
+// fused-plaquette partials (fixed slice, fixed order) and stores it beside its Polyakov
+// partial; the CTA that draws the last ticket then sums the gridDim.x slot pairs in index
+// order. Grid and slices depend on the lattice only: a given lattice always gives the same bits.
+struct StepTail {
+    const double* epart;  // [device] fused-plaquette partials of the sweep; NULL = no tail (plain Polyakov kernel)
+    size_t n_epart;
+    double scale_plaq, scale_poly;
+    double* slots;        // [device] 2 * gridDim.x doubles
+    unsigned* ticket;     // [device] zero between steps
+    double* dst;          // [device] 2 doubles (ignored when state != NULL)
+    RunState* state;      // su2_run: destination state->out[2*index..], then sweep and index advance
+};
+__device__ __forceinline__ void step_tail(const StepTail& tl, double poly_tot, double* red)
+{
+    __shared__ bool is_last;
+    const unsigned G = gridDim.x, b = blockIdx.x;
+    const size_t chunk = (tl.n_epart + G - 1) / G;
+    const size_t lo = (size_t)b * chunk, hi = (lo + chunk < tl.n_epart) ? lo + chunk : tl.n_epart;
+    double acc = 0.0;
+    for (size_t i = lo + threadIdx.x; i < hi; i += blockDim.x) acc += __ldcg(tl.epart + i);
+    const double ea = block_sum(acc, red);
+    if (threadIdx.x == 0) {
+        tl.slots[2 * b] = ea;
+        tl.slots[2 * b + 1] = poly_tot;
+        __threadfence();
+        is_last = atomicAdd(tl.ticket, 1u) == G - 1;
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    double sa = 0.0, sb = 0.0;
+    for (unsigned i = threadIdx.x; i < G; i += blockDim.x) {
+        sa += __ldcg(tl.slots + 2 * i);
+        sb += __ldcg(tl.slots + 2 * i + 1);
+    }
+    const double ta = block_sum(sa, red);
+    const double tb = block_sum(sb, red);
+    if (threadIdx.x == 0) {
+        double* dst = tl.state ? tl.state->out + 2 * (size_t)tl.state->index : tl.dst;
+        dst[0] = ta * tl.scale_plaq;
+        dst[1] = tb * tl.scale_poly;
+        *tl.ticket = 0u;
+        if (tl.state) {
+            tl.state->sweep += 1u;
+            tl.state->index += 1u;
+        }
+    }
+}
+
 // ------------------------------------------------------------------ Polyakov loop
 // one thread per spatial site; ordered product of the N_t time links [R11]
 template <typename Real>
 __global__ void __launch_bounds__(kBlock)
     polyakov_kernel(const typename LinkPtr<Real>::type* __restrict__ links, const Geom g,
-                    double* __restrict__ field, double* __restrict__ partials)
+                    double* __restrict__ field, double* __restrict__ partials, const StepTail tl)
 {
     typedef typename LinkPtr<Real>::type L;
     __shared__ double red[kBlock / 32];
     const uint32_t v3 = (uint32_t)g.n[0] * (uint32_t)g.n[1] * (uint32_t)g.n[2];
     const uint32_t s3 = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
+    // as the last kernel of a step it may be scheduled while sub-step (3,1) drains:
+    // every thread waits (the tail reads that kernel's partials), links are read through L2
+    grid_dep_wait();
+    grid_dep_launch();
     double val = 0.0;
     if (s3 < v3) {
         const uint32_t x = s3 % (uint32_t)g.n[0];
@@ -142,15 +198,19 @@ __global__ void __launch_bounds__(kBlock)
         const size_t vh = g.vh;
         const L* a0 = links + (size_t)(p0 * 4 + 3) * vh + (s3 >> 1);        // even t
         const L* a1 = links + (size_t)((1 - p0) * 4 + 3) * vh + (s3 >> 1);  // odd t
-        Quat<Real> prod = ldq(a0);
+        Quat<Real> prod = ldq_cg(a0);
         for (int t = 1; t < g.n[3]; ++t) {
-            const Quat<Real> u = ldq(((t & 1) ? a1 : a0) + (size_t)t * (size_t)g.st);
+            const Quat<Real> u = ldq_cg(((t & 1) ? a1 : a0) + (size_t)t * (size_t)g.st);
             prod = qmul<false, false>(prod, u);
         }
         val = (double)prod.a0;
         if (field) field[s3] = val;
     }
     const double tot = block_sum(val, red);
+    if (tl.epart) {
+        step_tail(tl, tot, red);
+        return;
+    }
     if (threadIdx.x == 0) partials[blockIdx.x] = tot;
 }
 
@@ -161,7 +221,7 @@ __global__ void __launch_bounds__(kBlock)
 template <typename Real, int S>
 __global__ void __launch_bounds__(kBlock)
     polyakov_split_kernel(const typename LinkPtr<Real>::type* __restrict__ links, const Geom g,
-                          double* __restrict__ field, double* __restrict__ partials)
+                          double* __restrict__ field, double* __restrict__ partials, const StepTail tl)
 {
     typedef typename LinkPtr<Real>::type L;
     constexpr int SITES = kBlock / S;
@@ -171,6 +231,8 @@ __global__ void __launch_bounds__(kBlock)
     const int seg = threadIdx.x / SITES, lane = threadIdx.x % SITES;
     const uint32_t s3 = blockIdx.x * (uint32_t)SITES + lane;
     const int len = g.n[3] / S, t0 = seg * len;
+    grid_dep_wait();
+    grid_dep_launch();
     if (s3 < v3) {
         const uint32_t x = s3 % (uint32_t)g.n[0];
         const uint32_t q = s3 / (uint32_t)g.n[0];
@@ -179,10 +241,10 @@ __global__ void __launch_bounds__(kBlock)
         const size_t vh = g.vh;
         const L* a0 = links + (size_t)(p0 * 4 + 3) * vh + (s3 >> 1);        // even t
         const L* a1 = links + (size_t)((1 - p0) * 4 + 3) * vh + (s3 >> 1);  // odd t
-        Quat<Real> prod = ldq(((t0 & 1) ? a1 : a0) + (size_t)t0 * (size_t)g.st);
+        Quat<Real> prod = ldq_cg(((t0 & 1) ? a1 : a0) + (size_t)t0 * (size_t)g.st);
 #pragma unroll 4
         for (int t = t0 + 1; t < t0 + len; ++t) {
-            const Quat<Real> u = ldq(((t & 1) ? a1 : a0) + (size_t)t * (size_t)g.st);
+            const Quat<Real> u = ldq_cg(((t & 1) ? a1 : a0) + (size_t)t * (size_t)g.st);
             prod = qmul<false, false>(prod, u);
         }
         part[seg][lane] = prod;
@@ -197,6 +259,10 @@ __global__ void __launch_bounds__(kBlock)
         if (field) field[s3] = val;
     }
     const double tot = block_sum(val, red);
+    if (tl.epart) {
+        step_tail(tl, tot, red);
+        return;
+    }
     if (threadIdx.x == 0) partials[blockIdx.x] = tot;
 }
 
@@ -309,66 +375,13 @@ int launch_plaquette(const void* links, const Geom& g, int precision, const Scra
     return 2;
 }
 
-// su2_run variants: destination and loop counters live in the device RunState
-__global__ void __launch_bounds__(1024)
-    final_sum_state_kernel(const double* __restrict__ partials, size_t n, double scale, RunState* __restrict__ state,
-                           int slot, int advance)
-{
-    __shared__ double red[32];
-    double acc = 0.0;
-    for (size_t i = threadIdx.x; i < n; i += 1024) acc += partials[i];
-    const double tot = block_sum(acc, red);
-    if (threadIdx.x == 0) {
-        state->out[2 * (size_t)state->index + slot] = tot * scale;
-        if (advance) {
-            state->sweep += 1u;
-            state->index += 1u;
-        }
-    }
-}
+// su2_run: the loop state the captured step reads and its last kernel advances
 __global__ void set_run_state_kernel(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index)
 {
     state->inv_beta = inv_beta;
     state->out = out;
     state->sweep = sweep;
     state->index = index;
-}
-// both observables of a step in one launch (one CTA, the two fixed-order sums one after the
-// other): dst = (plaquette, Polyakov loop); with `state` the destination is
-// state->out[2*index .. 2*index+1] and the loop counters advance (su2_run)
-__global__ void __launch_bounds__(1024)
-    final_sum2_kernel(const double* __restrict__ pa, size_t na, double sa, const double* __restrict__ pb, size_t nb,
-                      double sb, double* __restrict__ dst, RunState* __restrict__ state)
-{
-    __shared__ double red[32];
-    double acc = 0.0;
-    for (size_t i = threadIdx.x; i < na; i += 1024) acc += pa[i];
-    const double ta = block_sum(acc, red);
-    acc = 0.0;
-    for (size_t i = threadIdx.x; i < nb; i += 1024) acc += pb[i];
-    const double tb = block_sum(acc, red);
-    if (threadIdx.x == 0) {
-        if (state) dst = state->out + 2 * (size_t)state->index;
-        dst[0] = ta * sa;
-        dst[1] = tb * sb;
-        if (state) {
-            state->sweep += 1u;
-            state->index += 1u;
-        }
-    }
-}
-int launch_final_sum2(const double* pa, size_t na, double sa, const double* pb, size_t nb, double sb, double* dst,
-                      RunState* state, cudaStream_t st)
-{
-    final_sum2_kernel<<<1, 1024, 0, st>>>(pa, na, sa, pb, nb, sb, dst, state);
-    return 1;
-}
-
-int launch_final_sum_state(const double* partials, size_t n, double scale, RunState* state, int slot, bool advance,
-                           cudaStream_t st)
-{
-    final_sum_state_kernel<<<1, 1024, 0, st>>>(partials, n, scale, state, slot, advance ? 1 : 0);
-    return 1;
 }
 int launch_set_run_state(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index,
                          cudaStream_t st)
@@ -384,7 +397,8 @@ int launch_final_sum(const double* partials, size_t n, double scale, double* dev
 }
 
 template <typename Real>
-static unsigned launch_polyakov_t(const void* links, const Geom& g, const Scratch& sc, cudaStream_t st)
+static unsigned launch_polyakov_t(const void* links, const Geom& g, const Scratch& sc, const StepTail& tl,
+                                  bool overlap, cudaStream_t st)
 {
     typedef typename LinkPtr<Real>::type L;
     const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
@@ -393,24 +407,42 @@ static unsigned launch_polyakov_t(const void* links, const Geom& g, const Scratc
     const bool small = v3 < 148ull * 1024ull;
     if (small && nt >= 16 && nt % 4 == 0) {
         const unsigned grid = (unsigned)((v3 + kBlock / 4 - 1) / (kBlock / 4));
-        polyakov_split_kernel<Real, 4><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.field, sc.partials);
+        launch_ex(polyakov_split_kernel<Real, 4>, dim3(grid), dim3(kBlock), st, overlap, (const L*)links, g, sc.field,
+                  sc.partials, tl);
         return grid;
     }
     if (small && nt >= 8 && nt % 2 == 0) {
         const unsigned grid = (unsigned)((v3 + kBlock / 2 - 1) / (kBlock / 2));
-        polyakov_split_kernel<Real, 2><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.field, sc.partials);
+        launch_ex(polyakov_split_kernel<Real, 2>, dim3(grid), dim3(kBlock), st, overlap, (const L*)links, g, sc.field,
+                  sc.partials, tl);
         return grid;
     }
     const unsigned grid = blocks_for(v3);
-    polyakov_kernel<Real><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.field, sc.partials);
+    launch_ex(polyakov_kernel<Real>, dim3(grid), dim3(kBlock), st, overlap, (const L*)links, g, sc.field, sc.partials,
+              tl);
     return grid;
 }
 
 int launch_polyakov_partials(const void* links, const Geom& g, int precision, const Scratch& sc, size_t* n_partials,
                              cudaStream_t st)
 {
-    *n_partials = precision == 32 ? launch_polyakov_t<float>(links, g, sc, st)
-                                  : launch_polyakov_t<double>(links, g, sc, st);
+    const StepTail none = {};
+    *n_partials = precision == 32 ? launch_polyakov_t<float>(links, g, sc, none, false, st)
+                                  : launch_polyakov_t<double>(links, g, sc, none, false, st);
+    return 1;
+}
+
+// the last kernel of a step: Polyakov loop + both final sums (see step_tail)
+int launch_polyakov_step(const void* links, const Geom& g, int precision, const Scratch& sc, const double* epart,
+                         size_t n_epart, double scale_plaq, double* dev_dst, RunState* state, bool overlap,
+                         cudaStream_t st)
+{
+    const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
+    const StepTail tl = {epart, n_epart, scale_plaq, 1.0 / (double)v3, sc.slots, sc.ticket, dev_dst, state};
+    if (precision == 32)
+        launch_polyakov_t<float>(links, g, sc, tl, overlap, st);
+    else
+        launch_polyakov_t<double>(links, g, sc, tl, overlap, st);
     return 1;
 }
 
