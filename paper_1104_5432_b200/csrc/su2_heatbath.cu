@@ -202,7 +202,7 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
 #define HB_MINB_F32 8
 #endif
 #ifndef HB_MINB_F64
-#define HB_MINB_F64 8
+#define HB_MINB_F64 7
 #endif
 template <typename Real>
 struct MinBlocks {
