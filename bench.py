@@ -208,6 +208,9 @@ def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, 
 
     # extra (not the headline): the same `steps` steps as ONE su2_run call — the step captured as
     # a CUDA graph and replayed, no host work per step (matters on small lattices)
+    time.sleep(COOL_DOWN_S)  # same power state as the timed region above started from
+    lat.run(beta, warmup + steps, min(warmup, steps), obs)  # captures the graph
+    torch.cuda.synchronize()
     s2, e2 = ev(), ev()
     s2.record()
     lat.run(beta, warmup + steps, steps, obs)
@@ -427,7 +430,7 @@ def main():
         "init_ms": r["init_ms"], "plaquette_last": r["plaquette_last"], "polyakov_last": r["polyakov_last"],
         "su2_run": {"value": world * w.links / (r["ms_per_step_run"] * 1e-3), "unit": UNIT,
                     "ms_per_step": r["ms_per_step_run"],
-                    "what": "the same steps as one su2_run call (captured CUDA graph replayed), timed right after"},
+                    "what": "the same steps as one su2_run call (captured CUDA graph replayed), timed after the same cool-down"},
     }
 
     if not args.headline_only and rank == 0:

@@ -141,7 +141,7 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.epart, 3 * heatbath_ctas(g) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.field, v3 * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.out, (2 + kMaxR) * sizeof(double));
-    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.state, sizeof(RunState));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.state, kRunCopies * sizeof(RunState));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.slots, 2 * (v3 / 64 + 1) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.ticket, sizeof(unsigned));
     if (ce == cudaSuccess) ce = cudaMemset(lat->sc.ticket, 0, sizeof(unsigned));

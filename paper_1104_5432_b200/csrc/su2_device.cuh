@@ -350,25 +350,29 @@ struct M<double> {
 // step is replayed n times without touching its kernel parameters, so what changes from
 // step to step lives here. Written by set_run_state_kernel and advanced by the last
 // kernel of every step.
-struct RunState {
+struct __align__(32) RunState {
     double inv_beta;
-    double* out;      // [device] 2 doubles per step
     uint32_t sweep;   // sweep_idx of the current step
     uint32_t index;   // step number: results go to out[2*index], out[2*index+1]
+    double* out;      // [device] 2 doubles per step
+    uint64_t pad;
 };
-__device__ __forceinline__ uint32_t ld_cg_u32(const uint32_t* p)
+// Every thread of a sub-step reads (inv_beta, sweep). With one copy the 2^18 warps of a 64^4
+// launch would all address a single L2 sector, so the state is replicated: a CTA reads copy (CTA id mod kRunCopies), the last kernel
+// of a step advances all copies. Copy 0 is the one whose `out` and `index` are used.
+constexpr int kRunCopies = 1024;
+__device__ __forceinline__ const RunState* run_state_copy(const RunState* base)
 {
-    uint32_t v;
-    asm volatile("ld.global.cg.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
+    return base + ((blockIdx.x + 37u * blockIdx.y + 101u * blockIdx.z) & (uint32_t)(kRunCopies - 1));
 }
-__device__ __forceinline__ double ld_cg_f64(const double* p)
+// (inv_beta, sweep) in one 16-byte L2 load
+__device__ __forceinline__ void ld_run_state(const RunState* p, double& inv_beta, uint32_t& sweep)
 {
-    double v;
-    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
-    return v;
+    uint64_t a, b;
+    asm volatile("ld.global.cg.v2.u64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+    inv_beta = __longlong_as_double((long long)a);
+    sweep = (uint32_t)b;
 }
-
 // per-launch constants of the heat-bath kernels. The array bases are resolved on the
 // host so that a link address is base + 16*(32-bit index): one IMAD.WIDE per load.
 template <typename Real>

@@ -45,9 +45,22 @@ struct SiteIdx {
     int r;  // low bit of x
 };
 
+template <typename Real>
+__device__ __forceinline__ void run_state(const HbParams<Real>& hp, uint32_t& sweep, Real& inv_beta)
+{
+    sweep = hp.sweep;
+    inv_beta = hp.inv_beta;
+    if (hp.state) {  // su2_run: the captured graph's parameters are frozen, the loop state is not
+        double ib;
+        ld_run_state(run_state_copy(hp.state), ib, sweep);
+        inv_beta = (Real)ib;
+    }
+}
+
 // neighbour addressing (row 2) and the 18 loads (row 3, first half) of one site
 template <typename Real, int MU, int P>
-__device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const HbParams<Real>& hp, Staple18<Real>& q)
+__device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const HbParams<Real>& hp, Staple18<Real>& q,
+                                          uint32_t& sweep, Real& inv_beta)
 {
     typedef typename LinkPtr<Real>::type L;
     constexpr int DEP_NU = (P == 0) ? (MU + 3) % 4 : -1;
@@ -72,6 +85,9 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
         q.a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));             // U_nu(x+mu-nu)
         q.b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
         q.c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
+        // su2_run's loop state is fetched behind the first six link loads: its round trip then
+        // overlaps theirs instead of preceding them (the n = 0 Philox call needs `sweep`)
+        if (i == 0) run_state(hp, sweep, inv_beta);
     }
     return ix;
 }
@@ -171,17 +187,6 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
     return MEAS ? u.a0 * w.a0 - u.a1 * w.a1 - u.a2 * w.a2 - u.a3 * w.a3 : (Real)0;  // 1/2 Tr(U' w)
 }
 
-template <typename Real>
-__device__ __forceinline__ void run_state(const HbParams<Real>& hp, uint32_t& sweep, Real& inv_beta)
-{
-    sweep = hp.sweep;
-    inv_beta = hp.inv_beta;
-    if (hp.state) {  // su2_run: the captured graph's parameters are frozen, the loop state is not
-        sweep = ld_cg_u32(&hp.state->sweep);
-        inv_beta = (Real)ld_cg_f64(&hp.state->inv_beta);
-    }
-}
-
 template <typename Real, int MU, int P, bool MEAS, bool ALT>
 __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
                                               int* __restrict__ err)
@@ -190,9 +195,8 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     grid_dep_launch();  // ... so the next one may be scheduled behind this CTA
     uint32_t sweep;
     Real inv_beta;
-    run_state(hp, sweep, inv_beta);
     Staple18<Real> q;
-    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q);
+    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta);
     return update_link<Real, MU, P, MEAS, ALT>(q, ix, sweep, inv_beta, hp, kLogTab, err);
 }
 

@@ -167,11 +167,12 @@ __device__ __forceinline__ void step_tail(const StepTail& tl, double poly_tot, d
         dst[0] = ta * tl.scale_plaq;
         dst[1] = tb * tl.scale_poly;
         *tl.ticket = 0u;
-        if (tl.state) {
-            tl.state->sweep += 1u;
-            tl.state->index += 1u;
-        }
     }
+    if (tl.state)  // su2_run: advance every copy of the loop state (this CTA is the last one running)
+        for (int i = threadIdx.x; i < kRunCopies; i += blockDim.x) {
+            tl.state[i].sweep += 1u;
+            tl.state[i].index += 1u;
+        }
 }
 
 // ------------------------------------------------------------------ Polyakov loop
@@ -378,6 +379,7 @@ int launch_plaquette(const void* links, const Geom& g, int precision, const Scra
 // su2_run: the loop state the captured step reads and its last kernel advances
 __global__ void set_run_state_kernel(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index)
 {
+    state += blockIdx.x * blockDim.x + threadIdx.x;  // one thread per copy
     state->inv_beta = inv_beta;
     state->out = out;
     state->sweep = sweep;
@@ -386,7 +388,7 @@ __global__ void set_run_state_kernel(RunState* state, double inv_beta, double* o
 int launch_set_run_state(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index,
                          cudaStream_t st)
 {
-    set_run_state_kernel<<<1, 1, 0, st>>>(state, inv_beta, out, sweep, index);
+    set_run_state_kernel<<<kRunCopies / 256, 256, 0, st>>>(state, inv_beta, out, sweep, index);
     return 1;
 }
 
