@@ -92,3 +92,29 @@ def test_config2_polyakov_loop_rises_across_the_nt4_transition():
         lat.close()
     assert all(np.diff(plaq) > 0)
     assert absL[0] < 0.08 and absL[-1] > 0.25 and absL[-1] > 3 * absL[0], absL
+
+
+@pytest.mark.parametrize("method", ["auto", "creutz", "kp"])
+@pytest.mark.parametrize("prec", [32, 64])
+def test_strong_coupling_plaquette_with_every_draw(prec, method):
+    """A pin of the CUDA path that does not go through the oracle: at beta = 0.5 in D = 4 the
+    strong-coupling series gives <P> = u + O(u^5), u = I2(beta)/I1(beta) = 0.123718 (SURVEY.md §8(c)
+    pin table; the correction is ~1e-4). alpha = beta k ~ 1.2 here, so 'auto' runs Creutz's draw on
+    most links and KP on the rest; all three draws sample the same law."""
+    import torch
+    from scipy import special
+    import paper_1104_5432_b200 as pkg
+    dims, beta, ntherm, n = (16, 16, 16, 16), 0.5, 20, 300
+    lat = pkg.Lattice(dims, prec)
+    lat.init("hot", 41)
+    lat.set_draw(method)
+    obs = torch.zeros(2 * (ntherm + n), dtype=torch.float64, device="cuda")
+    lat.run(beta, 0, ntherm + n, obs)
+    lat.synchronize()
+    p = obs.cpu().numpy().reshape(-1, 2)[ntherm:, 0]
+    lat.close()
+    u = special.iv(2, beta) / special.iv(1, beta)
+    assert abs(u - 0.123718) < 1e-6
+    mean, err = _binned_error(p, 10)
+    assert err < 1e-4
+    assert abs(mean - u) < 3e-4 + 4 * err, (mean, err, u)
