@@ -57,10 +57,43 @@ __device__ __forceinline__ void run_state(const HbParams<Real>& hp, uint32_t& sw
     }
 }
 
+#ifdef HB_TMA  // tuning probe (never in the product build): the three unshifted U_nu(x) tiles of a CTA
+               // are staged through shared memory by TMA bulk copies (cp.async.bulk + mbarrier), one
+               // contiguous row of 2^LHX links per (y,z,t) of the tile; the other 15 loads stay LDGs.
+template <typename Real>
+struct TmaStage {
+    typename LinkPtr<Real>::type* buf;  // [3][blockDim.x]
+    uint64_t* bar;
+    int row_len;                        // links per contiguous row = 2^LHX
+};
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase)
+{
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)),
+        "r"(phase)
+        : "memory");
+}
+#endif
+
 // neighbour addressing (row 2) and the 18 loads (row 3, first half) of one site
 template <typename Real, int MU, int P>
 __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const HbParams<Real>& hp, Staple18<Real>& q,
-                                          uint32_t& sweep, Real& inv_beta)
+                                          uint32_t& sweep, Real& inv_beta
+#ifdef HB_TMA
+                                          ,
+                                          const TmaStage<Real>* tma = nullptr
+#endif
+)
 {
     typedef typename LinkPtr<Real>::type L;
     constexpr int DEP_NU = (P == 0) ? (MU + 3) % 4 : -1;
@@ -72,6 +105,25 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     const Nbr d = neighbours(g, c, ix.r);
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
     const uint32_t h_up = (uint32_t)(h + d.up[MU]);
+#ifdef HB_TMA
+    if (tma) {
+        const uint32_t row_bytes = (uint32_t)tma->row_len * (uint32_t)sizeof(L);
+        if (threadIdx.x == 0) {
+            uint64_t st_;
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 %0, [%1], %2;"
+                         : "=l"(st_)
+                         : "r"(smem_u32(tma->bar)), "r"(3u * blockDim.x * (uint32_t)sizeof(L))
+                         : "memory");
+        }
+        if ((threadIdx.x & (tma->row_len - 1)) == 0) {  // row leader: its h is the row start
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                const int nu = i + (i >= MU ? 1 : 0);
+                bulk_g2s(tma->buf + i * blockDim.x + threadIdx.x, hp.same[nu] + (uint32_t)h, row_bytes, tma->bar);
+            }
+        }
+    }
+#endif
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         const int nu = i + (i >= MU ? 1 : 0);
@@ -81,6 +133,9 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
         const uint32_t h_upnu = (uint32_t)(h + d.up[nu]);
         q.a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
         q.b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
+#ifdef HB_TMA
+        if (!tma)
+#endif
         q.cc[i] = ldq(s_nu + (uint32_t)h);                                  // U_nu(x)
         q.a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));             // U_nu(x+mu-nu)
         q.b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
@@ -89,6 +144,16 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
         // overlaps theirs instead of preceding them (the n = 0 Philox call needs `sweep`)
         if (i == 0) run_state(hp, sweep, inv_beta);
     }
+#ifdef HB_TMA
+    if (tma) {
+        mbar_wait(tma->bar, 0u);
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            const L v = tma->buf[i * blockDim.x + threadIdx.x];
+            q.cc[i] = {v.x, v.y, v.z, v.w};
+        }
+    }
+#endif
     return ix;
 }
 
@@ -189,14 +254,23 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
 
 template <typename Real, int MU, int P, bool MEAS, bool ALT>
 __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
-                                              int* __restrict__ err)
+                                              int* __restrict__ err
+#ifdef HB_TMA
+                                              ,
+                                              const TmaStage<Real>* tma = nullptr
+#endif
+)
 {
     grid_dep_wait();    // the preceding kernel of the stream has finished and flushed
     grid_dep_launch();  // ... so the next one may be scheduled behind this CTA
     uint32_t sweep;
     Real inv_beta;
     Staple18<Real> q;
+#ifdef HB_TMA
+    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, tma);
+#else
     const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta);
+#endif
     return update_link<Real, MU, P, MEAS, ALT>(q, ix, sweep, inv_beta, hp, kLogTab, err);
 }
 
@@ -224,7 +298,19 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::va
     heatbath_tiled_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
     const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z);
+#ifdef HB_TMA
+    __shared__ __align__(128) typename LinkPtr<Real>::type stage_buf[3 << (LHX + LY + LZ + LT)];
+    __shared__ __align__(8) uint64_t stage_bar;
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&stage_bar)) : "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();  // ahead of griddepcontrol.wait: overlaps the predecessor's tail
+    const TmaStage<Real> tma = {stage_buf, &stage_bar, 1 << LHX};
+    const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, err, &tma);
+#else
     const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, err);
+#endif
     if (MEAS) {  // one fp64 partial per CTA, fixed order
         __shared__ double red[kBlock / 32];
         const double tot = block_sum_end(e, red);
