@@ -57,12 +57,19 @@ __device__ __forceinline__ void run_state(const HbParams<Real>& hp, uint32_t& sw
     }
 }
 
-#ifdef HB_TMA  // tuning probe (never in the product build): the three unshifted U_nu(x) tiles of a CTA
-               // are staged through shared memory by TMA bulk copies (cp.async.bulk + mbarrier), one
-               // contiguous row of 2^LHX links per (y,z,t) of the tile; the other 15 loads stay LDGs.
+#ifdef HB_TMA  // tuning probe (never in the product build): HB_TMA is a mask of the link reads that are
+               // staged through shared memory by TMA bulk copies (cp.async.bulk + mbarrier) instead of
+               // LDGs: bit 0 U_nu(x), 1 U_nu(x-nu), 2 U_mu(x-nu), 3 U_nu(x+mu-nu), 4 U_mu(x+nu),
+               // 5 U_nu(x+mu), each for the three nu. A shifted tile of the CTA is 2^(LY+LZ+LT) contiguous
+               // rows of 2^LHX links (two pieces where a row wraps in x); the row's first thread copies it.
+enum { TMA_CC = 0, TMA_C2 = 1, TMA_B2 = 2, TMA_A2 = 3, TMA_B = 4, TMA_A = 5 };
+__host__ __device__ constexpr int tma_popc(int m) { return m ? (m & 1) + tma_popc(m >> 1) : 0; }
+__host__ __device__ constexpr bool tma_on(int type) { return ((HB_TMA) >> type) & 1; }
+__host__ __device__ constexpr int tma_slot(int type, int i) { return 3 * tma_popc((HB_TMA) & ((1 << type) - 1)) + i; }
+constexpr int kTmaSlots = 3 * tma_popc(HB_TMA);
 template <typename Real>
 struct TmaStage {
-    typename LinkPtr<Real>::type* buf;  // [3][blockDim.x]
+    typename LinkPtr<Real>::type* buf;  // [kTmaSlots][blockDim.x]
     uint64_t* bar;
     int row_len;                        // links per contiguous row = 2^LHX
 };
@@ -82,6 +89,21 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase)
         "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)),
         "r"(phase)
         : "memory");
+}
+// one row of a shifted tile: links hx0+sx .. hx0+sx+len-1 (mod nxh) of the row at `row` (its hx = 0 element)
+template <typename L>
+__device__ __forceinline__ void tma_row(L* dst, const L* row, int hx0, int sx, int len, int nxh, uint64_t* bar)
+{
+    const int start = hx0 + sx;
+    if (start < 0) {
+        bulk_g2s(dst, row + (nxh - 1), (uint32_t)sizeof(L), bar);
+        bulk_g2s(dst + 1, row, (uint32_t)((len - 1) * sizeof(L)), bar);
+    } else if (start + len > nxh) {
+        bulk_g2s(dst, row + start, (uint32_t)((len - 1) * sizeof(L)), bar);
+        bulk_g2s(dst + (len - 1), row, (uint32_t)sizeof(L), bar);
+    } else {
+        bulk_g2s(dst, row + start, (uint32_t)(len * sizeof(L)), bar);
+    }
 }
 #endif
 
@@ -107,22 +129,36 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     const uint32_t h_up = (uint32_t)(h + d.up[MU]);
 #ifdef HB_TMA
     if (tma) {
-        const uint32_t row_bytes = (uint32_t)tma->row_len * (uint32_t)sizeof(L);
         if (threadIdx.x == 0) {
             uint64_t st_;
             asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 %0, [%1], %2;"
                          : "=l"(st_)
-                         : "r"(smem_u32(tma->bar)), "r"(3u * blockDim.x * (uint32_t)sizeof(L))
+                         : "r"(smem_u32(tma->bar)), "r"((uint32_t)kTmaSlots * blockDim.x * (uint32_t)sizeof(L))
                          : "memory");
         }
-        if ((threadIdx.x & (tma->row_len - 1)) == 0) {  // row leader: its h is the row start
+        if ((threadIdx.x & (tma->row_len - 1)) == 0) {  // row leader (c.hx = first hx of the tile)
+            const int row0 = h - c.hx;                   // the row's hx = 0 element
+            const int sx_up = ix.r ? 1 : 0, sx_dn = ix.r ? 0 : -1;  // half-index shift of x+1 / x-1
+            const int mu_nonx = (MU == 0) ? 0 : d.up[MU], mu_sx = (MU == 0) ? sx_up : 0;
 #pragma unroll
             for (int i = 0; i < 3; ++i) {
                 const int nu = i + (i >= MU ? 1 : 0);
-                bulk_g2s(tma->buf + i * blockDim.x + threadIdx.x, hp.same[nu] + (uint32_t)h, row_bytes, tma->bar);
+                const int up_nonx = (nu == 0) ? 0 : d.up[nu], up_sx = (nu == 0) ? sx_up : 0;
+                const int dn_nonx = (nu == 0) ? 0 : d.dn[nu], dn_sx = (nu == 0) ? sx_dn : 0;
+                L* base = tma->buf + threadIdx.x;
+                const int n = tma->row_len, nbx = (int)blockDim.x;
+                if (tma_on(TMA_CC)) tma_row(base + tma_slot(TMA_CC, i) * nbx, hp.same[nu] + row0, c.hx, 0, n, g.nxh, tma->bar);
+                if (tma_on(TMA_C2)) tma_row(base + tma_slot(TMA_C2, i) * nbx, hp.oppo[nu] + (row0 + dn_nonx), c.hx, dn_sx, n, g.nxh, tma->bar);
+                if (tma_on(TMA_B2)) tma_row(base + tma_slot(TMA_B2, i) * nbx, o_mu + (row0 + dn_nonx), c.hx, dn_sx, n, g.nxh, tma->bar);
+                if (tma_on(TMA_A2)) tma_row(base + tma_slot(TMA_A2, i) * nbx, hp.same[nu] + (row0 + mu_nonx + dn_nonx), c.hx, mu_sx + dn_sx, n, g.nxh, tma->bar);
+                if (tma_on(TMA_B)) tma_row(base + tma_slot(TMA_B, i) * nbx, o_mu + (row0 + up_nonx), c.hx, up_sx, n, g.nxh, tma->bar);
+                if (tma_on(TMA_A)) tma_row(base + tma_slot(TMA_A, i) * nbx, hp.oppo[nu] + (row0 + mu_nonx), c.hx, mu_sx, n, g.nxh, tma->bar);
             }
         }
     }
+#define TMA_SKIP(type) if (!(tma && tma_on(type)))
+#else
+#define TMA_SKIP(type)
 #endif
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
@@ -131,15 +167,12 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
         const L* o_nu = hp.oppo[nu];
         const uint32_t h_dn = (uint32_t)(h + d.dn[nu]);
         const uint32_t h_upnu = (uint32_t)(h + d.up[nu]);
-        q.a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
-        q.b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
-#ifdef HB_TMA
-        if (!tma)
-#endif
-        q.cc[i] = ldq(s_nu + (uint32_t)h);                                  // U_nu(x)
-        q.a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));             // U_nu(x+mu-nu)
-        q.b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
-        q.c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
+        TMA_SKIP(TMA_A) q.a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
+        TMA_SKIP(TMA_B) q.b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
+        TMA_SKIP(TMA_CC) q.cc[i] = ldq(s_nu + (uint32_t)h);                                  // U_nu(x)
+        TMA_SKIP(TMA_A2) q.a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));             // U_nu(x+mu-nu)
+        TMA_SKIP(TMA_B2) q.b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
+        TMA_SKIP(TMA_C2) q.c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
         // su2_run's loop state is fetched behind the first six link loads: its round trip then
         // overlaps theirs instead of preceding them (the n = 0 Philox call needs `sweep`)
         if (i == 0) run_state(hp, sweep, inv_beta);
@@ -147,10 +180,20 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
 #ifdef HB_TMA
     if (tma) {
         mbar_wait(tma->bar, 0u);
+        const L* base = tma->buf + threadIdx.x;
+        const int nbx = (int)blockDim.x;
+        auto rd = [&](int type, int i) {
+            const L v = base[tma_slot(type, i) * nbx];
+            return Quat<Real>{v.x, v.y, v.z, v.w};
+        };
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-            const L v = tma->buf[i * blockDim.x + threadIdx.x];
-            q.cc[i] = {v.x, v.y, v.z, v.w};
+            if (tma_on(TMA_CC)) q.cc[i] = rd(TMA_CC, i);
+            if (tma_on(TMA_C2)) q.c2[i] = rd(TMA_C2, i);
+            if (tma_on(TMA_B2)) q.b2[i] = rd(TMA_B2, i);
+            if (tma_on(TMA_A2)) q.a2[i] = rd(TMA_A2, i);
+            if (tma_on(TMA_B)) q.b[i] = rd(TMA_B, i);
+            if (tma_on(TMA_A)) q.a[i] = rd(TMA_A, i);
         }
     }
 #endif
@@ -299,7 +342,7 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::va
 {
     const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z);
 #ifdef HB_TMA
-    __shared__ __align__(128) typename LinkPtr<Real>::type stage_buf[3 << (LHX + LY + LZ + LT)];
+    __shared__ __align__(128) typename LinkPtr<Real>::type stage_buf[kTmaSlots << (LHX + LY + LZ + LT)];
     __shared__ __align__(8) uint64_t stage_bar;
     if (threadIdx.x == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&stage_bar)) : "memory");
