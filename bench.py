@@ -231,6 +231,35 @@ def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, 
     return res
 
 
+def time_aux(pkg, torch, workloads):
+    """Not part of the metric: the finite-temperature configs through su2_run (one call, CUDA graph
+    replay) and the Polyakov-loop correlator (S8(f) NEXT-1) on BASELINE config 4, wall clock."""
+    out = {}
+    for name, prec, beta, n in (("C2_16^3x4", 32, 2.4, 200), ("C4_48^3x8", 64, 2.5, 100)):
+        w = workloads.BY_NAME[name]
+        lat = pkg.Lattice(w.dims, prec)
+        lat.init(w.start, w.seed)
+        obs = torch.zeros(2 * n, dtype=torch.float64, device=lat.device)
+        lat.run(beta, 0, 10, obs)
+        lat.synchronize()
+        t0 = time.perf_counter()
+        lat.run(beta, 10, n, obs)
+        lat.synchronize()
+        dt = time.perf_counter() - t0
+        rec = {"su2_run_us_per_step": dt / n * 1e6, "value": w.links * n / dt, "unit": UNIT, "beta": beta,
+               "precision": prec, "steps": n}
+        if name.startswith("C4"):
+            lat.polyakov_correlator(24)
+            t0 = time.perf_counter()
+            for _ in range(10):
+                c = lat.polyakov_correlator(24)
+            rec["correlator_r1_24_us_per_call"] = (time.perf_counter() - t0) / 10 * 1e6
+            rec["correlator_r1"] = float(c[0])
+        out[name] = rec
+        lat.close()
+    return out
+
+
 def time_e2e(pkg, torch, w, prec, beta, steps, warmup, seed):
     """Same step through the C-ABI with HOST buffers: every step copies the input
     configuration host->device (su2_set_links, pinned), runs sweep + plaquette +
@@ -454,6 +483,7 @@ def main():
                 "su2_run_ms_per_step": rr["ms_per_step_run"],
             }
         line["workloads"] = others
+        line["aux"] = time_aux(pkg, torch, workloads)
         line["e2e"] = time_e2e(pkg, torch, w, prec, args.beta, args.e2e_steps, 1, args.seed)
         slab = OracleSlab(w, prec, args.beta, args.seed, args.cpu_baseline_seconds)
         v, sec, n, _, _ = slab.step()
