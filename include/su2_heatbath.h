@@ -164,6 +164,36 @@ SU2_API int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_t s
  * Asynchronous. Errors: SU2_EARG (beta, NULL dev_out), SU2_ESTATE, SU2_ECUDA. */
 SU2_API int su2_run(su2_lattice* lat, double beta, uint32_t sweep_idx0, uint32_t n_steps, double* dev_out);
 
+/* S8(f) NEXT-2: replica batches. The paper's production mode is many small finite-temperature
+ * lattices, one per coupling (a beta scan per N_t); a 16^3 x 4 sub-step is 64 CTAs on a
+ * 148-SM GPU. A batch handle holds n_replicas configurations of the same geometry and precision, one
+ * after the other in device memory (replica r at byte offset r * su2_lattice_bytes(...)), and
+ * su2_batch_sweep_measure updates all of them with the same 9 launches a single lattice takes, each
+ * replica with its own beta and its own seed (its Philox streams are those of a single lattice with that
+ * seed).
+ *   n_replicas >= 1; n_replicas * 4V < 2^32; (N_z/2 * N_t-tiles) * n_replicas <= 65535.
+ * Every single-lattice call (init, sweep, measure, correlator, get/set_links, run ...) works on a batch
+ * handle and acts on the SELECTED replica (0 after create). The _external form takes caller-owned
+ * memory of n_replicas * su2_lattice_bytes(...) bytes. */
+SU2_API int su2_lattice_create_batch(int Nx, int Ny, int Nz, int Nt, int precision, int n_replicas,
+                                     su2_lattice** out);
+SU2_API int su2_lattice_create_batch_external(int Nx, int Ny, int Nz, int Nt, int precision, int n_replicas,
+                                              void* dev_links, size_t bytes, void* cuda_stream, su2_lattice** out);
+/* Number of replicas of the handle (1 for su2_lattice_create); 0 for NULL. */
+SU2_API int su2_replicas(const su2_lattice* lat);
+/* Make replica `replica` the one the single-lattice calls act on. Errors: SU2_EARG. */
+SU2_API int su2_select_replica(su2_lattice* lat, int replica);
+/* su2_init of every replica: replica r from seeds[r] ([host], n_replicas values). Asynchronous. */
+SU2_API int su2_batch_init(su2_lattice* lat, int start, const uint64_t* seeds);
+/* One step (heat-bath sweep [R4], mean plaquette [R10], Polyakov loop [R11]) of every replica:
+ * replica r at coupling betas[r] ([host], n_replicas values), Philox counter word sweep_idx for all.
+ * Results at dev_out[2*(index*n_replicas + r)], dev_out[2*(index*n_replicas + r) + 1] ([device]).
+ * The draw is the handle's (su2_set_draw). Asynchronous, except that a change of betas or seeds since
+ * the previous call first waits for the stream. Errors: SU2_EARG, SU2_ESTATE (a replica not
+ * initialised), SU2_ECUDA. */
+SU2_API int su2_batch_sweep_measure(su2_lattice* lat, const double* betas, uint32_t sweep_idx, double* dev_out,
+                                    size_t index);
+
 /* NEXT-1 (eq. 3): on-axis Polyakov-loop correlator
  * C(r) = < l(x) l(x + r e_i) >, averaged over all spatial x and the 3 spatial axes i,
  * r = 1..rmax (rmax <= min spatial extent / 2), l(x) = 1/2 Tr L(x) (real in SU(2)).

@@ -29,6 +29,13 @@ _SIGNATURES = {
     "su2_lattice_create": (C.c_int, [C.c_int] * 5 + [C.POINTER(C.c_void_p)]),
     "su2_lattice_create_external": (C.c_int, [C.c_int] * 5 + [C.c_void_p, C.c_size_t, C.c_void_p,
                                                              C.POINTER(C.c_void_p)]),
+    "su2_lattice_create_batch": (C.c_int, [C.c_int] * 6 + [C.POINTER(C.c_void_p)]),
+    "su2_lattice_create_batch_external": (C.c_int, [C.c_int] * 6 + [C.c_void_p, C.c_size_t, C.c_void_p,
+                                                                    C.POINTER(C.c_void_p)]),
+    "su2_replicas": (C.c_int, [C.c_void_p]),
+    "su2_select_replica": (C.c_int, [C.c_void_p, C.c_int]),
+    "su2_batch_init": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "su2_batch_sweep_measure": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_size_t]),
     "su2_lattice_destroy": (C.c_int, [C.c_void_p]),
     "su2_set_stream": (C.c_int, [C.c_void_p, C.c_void_p]),
     "su2_init": (C.c_int, [C.c_void_p, C.c_int, C.c_uint64]),
@@ -103,6 +110,37 @@ def su2_lattice_create_external(Nx, Ny, Nz, Nt, precision, dev_ptr, nbytes, cuda
     _check(lib().su2_lattice_create_external(Nx, Ny, Nz, Nt, precision, C.c_void_p(dev_ptr), nbytes,
                                              C.c_void_p(cuda_stream), C.byref(h)))
     return h
+
+
+def su2_lattice_create_batch(Nx, Ny, Nz, Nt, precision, n_replicas):
+    h = C.c_void_p()
+    _check(lib().su2_lattice_create_batch(Nx, Ny, Nz, Nt, precision, n_replicas, C.byref(h)))
+    return h
+
+
+def su2_lattice_create_batch_external(Nx, Ny, Nz, Nt, precision, n_replicas, dev_ptr, nbytes, cuda_stream=0):
+    h = C.c_void_p()
+    _check(lib().su2_lattice_create_batch_external(Nx, Ny, Nz, Nt, precision, n_replicas, C.c_void_p(dev_ptr), nbytes,
+                                                   C.c_void_p(cuda_stream), C.byref(h)))
+    return h
+
+
+def su2_replicas(h):
+    return lib().su2_replicas(h)
+
+
+def su2_select_replica(h, replica):
+    _check(lib().su2_select_replica(h, replica), h)
+
+
+def su2_batch_init(h, start, seeds):
+    a = np.ascontiguousarray(seeds, dtype=np.uint64)
+    _check(lib().su2_batch_init(h, start, C.c_void_p(a.ctypes.data)), h)
+
+
+def su2_batch_sweep_measure(h, betas, sweep_idx, dev_out_ptr, index):
+    a = np.ascontiguousarray(betas, dtype=np.float64)
+    _check(lib().su2_batch_sweep_measure(h, C.c_void_p(a.ctypes.data), sweep_idx, C.c_void_p(dev_out_ptr), index), h)
 
 
 def su2_lattice_destroy(h):
@@ -194,7 +232,7 @@ class Lattice:
     tensor (PyTorch owns the memory; the library borrows it), work runs on torch's
     current stream at construction time."""
 
-    def __init__(self, dims, precision=64, device="cuda:0"):
+    def __init__(self, dims, precision=64, device="cuda:0", replicas=1):
         import torch
 
         if not torch.cuda.is_available():
@@ -208,10 +246,16 @@ class Lattice:
             raise SU2Error(SU2_EARG, "extents must be even and >= 2, V < 2^32, precision 32 or 64")
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        self.storage = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.replicas = int(replicas)
+        self.storage = torch.empty(nbytes * self.replicas, dtype=torch.uint8, device=self.device)
         self.stream = torch.cuda.current_stream(self.device)
-        self.h = su2_lattice_create_external(Nx, Ny, Nz, Nt, self.precision, self.storage.data_ptr(), nbytes,
-                                             self.stream.cuda_stream)
+        if self.replicas == 1:
+            self.h = su2_lattice_create_external(Nx, Ny, Nz, Nt, self.precision, self.storage.data_ptr(), nbytes,
+                                                 self.stream.cuda_stream)
+        else:  # a batch of configurations updated together (su2_batch_*); other calls act on the selected one
+            self.h = su2_lattice_create_batch_external(Nx, Ny, Nz, Nt, self.precision, self.replicas,
+                                                       self.storage.data_ptr(), nbytes * self.replicas,
+                                                       self.stream.cuda_stream)
         self.volume = Nx * Ny * Nz * Nt
         self.nlinks = 4 * self.volume
 
@@ -231,6 +275,17 @@ class Lattice:
 
     def set_seed(self, seed):
         su2_set_seed(self.h, seed)
+
+    def select(self, replica):
+        su2_select_replica(self.h, replica)
+
+    def batch_init(self, start, seeds):
+        su2_batch_init(self.h, {"cold": SU2_START_COLD, "hot": SU2_START_HOT}[start], seeds)
+
+    def batch_sweep_measure(self, betas, sweep_idx, dev_out, index):
+        """dev_out: float64 device tensor; step `index` of replica r lands at [2*(index*replicas + r) + {0,1}]."""
+        assert len(betas) == self.replicas and dev_out.numel() >= 2 * self.replicas * (index + 1)
+        su2_batch_sweep_measure(self.h, betas, sweep_idx, dev_out.data_ptr(), index)
 
     def set_draw(self, method):
         su2_set_draw(self.h, {"kp": SU2_DRAW_KP, "auto": SU2_DRAW_AUTO, "creutz": SU2_DRAW_CREUTZ}[method])

@@ -31,6 +31,14 @@ struct su2_lattice {
     cudaGraphExec_t run_exec;
     bool run_graphs;   // SU2HB_NO_GRAPH=1 disables (A/B timing only)
     double creutz_below;  // [R15] su2_set_draw: 0 (KP), SU2_ALPHA_C (auto) or +inf (Creutz)
+    // replica batch: nrep configurations one after the other from links_base; `links`,
+    // `seed` and `initialised` are those of the selected replica (single-lattice calls act on it)
+    int nrep, selected;
+    void* links_base;
+    size_t rep_bytes;
+    uint64_t* rep_seed;        // [host] nrep
+    unsigned char* rep_init;   // [host] nrep
+    RepParams* rep_host;       // [host] nrep: what sc.reps holds
     void* stage;       // canonical-order staging buffer of su2_get_links / su2_set_links (lazy, kept)
     int sticky;  // sticky error code
     char msg[256];
@@ -97,13 +105,16 @@ extern "C" size_t su2_lattice_bytes(int Nx, int Ny, int Nz, int Nt, int precisio
     return (size_t)Nx * Ny * Nz * Nt * 4 * 4 * (precision == 32 ? sizeof(float) : sizeof(double));
 }
 
-static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_links, size_t bytes, void* stream,
-                       bool external, su2_lattice** out)
+static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, int nrep, void* dev_links, size_t bytes,
+                       void* stream, bool external, su2_lattice** out)
 {
     if (!out) return SU2_EARG;
     *out = nullptr;
     if (!valid_dims(Nx, Ny, Nz, Nt, precision)) return SU2_EARG;
-    const size_t need = su2_lattice_bytes(Nx, Ny, Nz, Nt, precision);
+    // a batch indexes every link of every replica with 32 bits and puts the replica in grid y / z
+    if (nrep < 1 || nrep > 65535 || (uint64_t)nrep * 4ull * Nx * Ny * Nz * Nt >= (1ull << 32)) return SU2_EARG;
+    const size_t rep_bytes = su2_lattice_bytes(Nx, Ny, Nz, Nt, precision);
+    const size_t need = rep_bytes * (size_t)nrep;
     if (external && (!dev_links || bytes < need || ((uintptr_t)dev_links & 31))) return SU2_EARG;
 
     su2_lattice* lat = new (std::nothrow) su2_lattice;
@@ -121,6 +132,12 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
     g.wup[2] = -(Nz - 1) * g.sz;
     g.wup[3] = -(Nt - 1) * g.st;
     choose_tiling(g);
+    if (g.tile >= 0 && (uint64_t)g.nb[2] * g.nb[3] * nrep > 65535) {  // grid z holds (replica, z-t tile)
+        delete lat;
+        return SU2_EARG;
+    }
+    lat->nrep = nrep;
+    lat->rep_bytes = rep_bytes;
     lat->precision = precision;
     lat->last_substep = -1;
     {
@@ -132,19 +149,28 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
     lat->stream = (cudaStream_t)stream;
     lat->owns_links = !external;
     lat->links = dev_links;
+    lat->rep_seed = (uint64_t*)calloc((size_t)nrep, sizeof(uint64_t));
+    lat->rep_init = (unsigned char*)calloc((size_t)nrep, 1);
+    lat->rep_host = (RepParams*)calloc((size_t)nrep, sizeof(RepParams));
+    if (!lat->rep_seed || !lat->rep_init || !lat->rep_host) {
+        su2_lattice_destroy(lat);
+        return SU2_EALLOC;
+    }
 
     cudaError_t ce = cudaSuccess;
     if (!external) ce = cudaMalloc(&lat->links, need);
     const uint64_t v3 = (uint64_t)Nx * Ny * Nz;
     lat->sc.n_partials = partials_needed(g);
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.partials, lat->sc.n_partials * sizeof(double));
-    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.epart, 3 * heatbath_ctas(g) * sizeof(double));
-    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.field, v3 * sizeof(double));
+    lat->links_base = lat->links;
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.epart, (size_t)nrep * 3 * heatbath_ctas(g) * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.field, (size_t)nrep * v3 * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.reps, (size_t)nrep * sizeof(RepParams));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.out, (2 + kMaxR) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.state, kRunCopies * sizeof(RunState));
-    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.slots, 2 * (v3 / 64 + 1) * sizeof(double));
-    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.ticket, sizeof(unsigned));
-    if (ce == cudaSuccess) ce = cudaMemset(lat->sc.ticket, 0, sizeof(unsigned));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.slots, (size_t)nrep * 2 * (v3 / 64 + 1) * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.ticket, (size_t)nrep * sizeof(unsigned));
+    if (ce == cudaSuccess) ce = cudaMemset(lat->sc.ticket, 0, (size_t)nrep * sizeof(unsigned));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.err, sizeof(int));
     if (ce == cudaSuccess) ce = cudaMemset(lat->sc.err, 0, sizeof(int));
     if (ce != cudaSuccess) {
@@ -159,19 +185,36 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_
 
 extern "C" int su2_lattice_create(int Nx, int Ny, int Nz, int Nt, int precision, su2_lattice** out)
 {
-    return create_impl(Nx, Ny, Nz, Nt, precision, nullptr, 0, nullptr, false, out);
+    return create_impl(Nx, Ny, Nz, Nt, precision, 1, nullptr, 0, nullptr, false, out);
+}
+
+extern "C" int su2_lattice_create_batch(int Nx, int Ny, int Nz, int Nt, int precision, int n_replicas,
+                                        su2_lattice** out)
+{
+    return create_impl(Nx, Ny, Nz, Nt, precision, n_replicas, nullptr, 0, nullptr, false, out);
+}
+
+extern "C" int su2_lattice_create_batch_external(int Nx, int Ny, int Nz, int Nt, int precision, int n_replicas,
+                                                 void* dev_links, size_t bytes, void* cuda_stream, su2_lattice** out)
+{
+    return create_impl(Nx, Ny, Nz, Nt, precision, n_replicas, dev_links, bytes, cuda_stream, true, out);
 }
 
 extern "C" int su2_lattice_create_external(int Nx, int Ny, int Nz, int Nt, int precision, void* dev_links,
                                            size_t bytes, void* cuda_stream, su2_lattice** out)
 {
-    return create_impl(Nx, Ny, Nz, Nt, precision, dev_links, bytes, cuda_stream, true, out);
+    return create_impl(Nx, Ny, Nz, Nt, precision, 1, dev_links, bytes, cuda_stream, true, out);
 }
 
 extern "C" int su2_lattice_destroy(su2_lattice* lat)
 {
     if (!lat) return SU2_OK;
-    if (lat->owns_links && lat->links) cudaFree(lat->links);
+    if (lat->owns_links && lat->links_base) cudaFree(lat->links_base);
+    else if (lat->owns_links && lat->links) cudaFree(lat->links);
+    if (lat->sc.reps) cudaFree(lat->sc.reps);
+    free(lat->rep_seed);
+    free(lat->rep_init);
+    free(lat->rep_host);
     if (lat->sc.partials) cudaFree(lat->sc.partials);
     if (lat->sc.epart) cudaFree(lat->sc.epart);
     if (lat->sc.field) cudaFree(lat->sc.field);
@@ -206,6 +249,8 @@ extern "C" int su2_init(su2_lattice* lat, int start, uint64_t seed)
     CK(lat, cudaGetLastError());
     lat->seed = seed;
     lat->initialised = true;
+    lat->rep_seed[lat->selected] = seed;
+    lat->rep_init[lat->selected] = 1;
     return SU2_OK;
 }
 
@@ -213,6 +258,91 @@ extern "C" int su2_set_seed(su2_lattice* lat, uint64_t seed)
 {
     ENTER(lat);
     lat->seed = seed;
+    lat->rep_seed[lat->selected] = seed;
+    return SU2_OK;
+}
+
+extern "C" int su2_replicas(const su2_lattice* lat) { return lat ? lat->nrep : 0; }
+
+static void drop_run_graph(su2_lattice* lat)
+{
+    if (lat->run_exec) {  // the captured step holds pointers into the replica selected at capture
+        cudaStreamSynchronize(lat->run_stream);
+        cudaGraphExecDestroy(lat->run_exec);
+        lat->run_exec = nullptr;
+    }
+}
+
+extern "C" int su2_select_replica(su2_lattice* lat, int replica)
+{
+    ENTER(lat);
+    NOT_A_SUBSTEP(lat);
+    if (replica < 0 || replica >= lat->nrep) return fail(lat, SU2_EARG, "su2_select_replica: no such replica");
+    if (replica != lat->selected) drop_run_graph(lat);
+    lat->selected = replica;
+    lat->links = (char*)lat->links_base + (size_t)replica * lat->rep_bytes;
+    lat->seed = lat->rep_seed[replica];
+    lat->initialised = lat->rep_init[replica] != 0;
+    return SU2_OK;
+}
+
+extern "C" int su2_batch_init(su2_lattice* lat, int start, const uint64_t* seeds)
+{
+    ENTER(lat);
+    NOT_A_SUBSTEP(lat);
+    if (start != SU2_START_COLD && start != SU2_START_HOT) return fail(lat, SU2_EARG, "su2_batch_init: bad start");
+    if (!seeds) return fail(lat, SU2_EARG, "su2_batch_init: NULL seeds");
+    for (int r = 0; r < lat->nrep; ++r) {
+        lat->launches += launch_init((char*)lat->links_base + (size_t)r * lat->rep_bytes, lat->g, lat->precision, start,
+                                     seeds[r], lat->stream);
+        lat->rep_seed[r] = seeds[r];
+        lat->rep_init[r] = 1;
+    }
+    CK(lat, cudaGetLastError());
+    lat->seed = lat->rep_seed[lat->selected];
+    lat->initialised = true;
+    return SU2_OK;
+}
+
+// One step of every replica in 9 launches: the 8 sub-steps over the whole batch (ALT
+// kernels, replica = leading part of the grid, 1/beta and seed per replica from device memory), then
+// the Polyakov kernel with one step tail per replica.
+extern "C" int su2_batch_sweep_measure(su2_lattice* lat, const double* betas, uint32_t sweep_idx, double* dev_out,
+                                       size_t index)
+{
+    ENTER(lat);
+    NOT_A_SUBSTEP(lat);
+    if (!betas || !dev_out) return fail(lat, SU2_EARG, "su2_batch_sweep_measure: NULL argument");
+    bool changed = false;
+    for (int r = 0; r < lat->nrep; ++r) {
+        if (!(betas[r] > 0.0) || !isfinite(betas[r])) return fail(lat, SU2_EARG, "beta must be finite and > 0");
+        if (!lat->rep_init[r]) return fail(lat, SU2_ESTATE, "a replica of the batch is not initialised");
+        const RepParams rp = {1.0 / betas[r], lat->rep_seed[r]};
+        changed = changed || rp.inv_beta != lat->rep_host[r].inv_beta || rp.seed != lat->rep_host[r].seed;
+        lat->rep_host[r] = rp;
+    }
+    if (changed) {  // rare: the kernels of earlier steps must have read the old values first
+        CK(lat, cudaStreamSynchronize(lat->stream));
+        CK(lat, cudaMemcpyAsync(lat->sc.reps, lat->rep_host, (size_t)lat->nrep * sizeof(RepParams),
+                                cudaMemcpyHostToDevice, lat->stream));
+    }
+    const size_t ctas = heatbath_ctas(lat->g);
+    int prev = -1;
+    for (int mu = 0; mu < 4; ++mu)
+        for (int p = 0; p < 2; ++p) {
+            const int idx = 2 * mu + p;
+            const bool overlap = lat->pdl && prev == (idx + 7) % 8;
+            lat->launches += launch_heatbath_substep(
+                lat->links_base, lat->g, lat->precision, mu, p, 1.0, lat->creutz_below, 0, sweep_idx, lat->sc.err,
+                (p == 1 && mu >= 1) ? lat->sc.epart + (mu - 1) * ctas : nullptr, nullptr, overlap, lat->stream,
+                lat->sc.reps, lat->nrep);
+            prev = idx;
+        }
+    lat->launches += launch_polyakov_step(lat->links_base, lat->g, lat->precision, lat->sc, lat->sc.epart, 3 * ctas,
+                                          1.0 / (6.0 * 2.0 * (double)lat->g.vh),
+                                          dev_out + 2 * index * (size_t)lat->nrep, nullptr, lat->pdl, lat->stream,
+                                          lat->nrep);
+    CK(lat, cudaGetLastError());
     return SU2_OK;
 }
 
@@ -474,6 +604,7 @@ extern "C" int su2_set_links(su2_lattice* lat, const void* host_src, size_t byte
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(lat->stream);
     if (ce != cudaSuccess) return fail(lat, SU2_ECUDA, "su2_set_links", ce);
     lat->initialised = true;
+    lat->rep_init[lat->selected] = 1;
     return SU2_OK;
 }
 

@@ -373,6 +373,18 @@ __device__ __forceinline__ void ld_run_state(const RunState* p, double& inv_beta
     inv_beta = __longlong_as_double((long long)a);
     sweep = (uint32_t)b;
 }
+// per-replica inputs of a batched launch
+struct __align__(16) RepParams {
+    double inv_beta;
+    uint64_t seed;
+};
+// what a thread needs to know about its replica; all zero for a single lattice
+struct RepCtx {
+    uint32_t rep;   // replica index
+    uint32_t hoff;  // rep * rep_stride: added to every link index
+    uint32_t k0, k1;  // Philox key words when the keys are not the launch's expanded ones
+};
+
 // per-launch constants of the heat-bath kernels. The array bases are resolved on the
 // host so that a link address is base + 16*(32-bit index): one IMAD.WIDE per load.
 template <typename Real>
@@ -386,6 +398,12 @@ struct __align__(16) HbParams {
     Real inv_beta;
     uint32_t sweep;
     Real creutz_below;  // [R15] ALT kernels: Creutz's draw where alpha < this (0 = never, +inf = always)
+    // replica batch (ALT kernels only): R configurations of the same geometry, one after
+    // the other in memory, updated by one launch; replica index = leading part of the grid
+    const RepParams* reps;  // [device] per-replica 1/beta and seed; NULL = single lattice
+    uint32_t rep_stride;    // links of one configuration: 8 * V/2
+    uint32_t nzt;           // tiled launch: CTAs along grid z per replica (nb2 * nb3)
+    uint32_t epart_stride;  // fused-plaquette partials per replica (3 * CTAs of one replica)
 };
 
 // [R9] Shoemake: uniform unit quaternion from three uniforms

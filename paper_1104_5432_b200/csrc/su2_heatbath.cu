@@ -41,8 +41,9 @@ struct Staple18 {  // the 18 links of one staple sum, per direction nu != mu (i 
     Quat<Real> a[3], b[3], cc[3], a2[3], b2[3], c2[3];
 };
 struct SiteIdx {
-    int h;  // half-index of the site
-    int r;  // low bit of x
+    int h;   // half-index of the site
+    int r;   // low bit of x
+    int ha;  // h + the replica's offset: index into the link arrays
 };
 
 template <typename Real>
@@ -110,7 +111,7 @@ __device__ __forceinline__ void tma_row(L* dst, const L* row, int hx0, int sx, i
 // neighbour addressing (row 2) and the 18 loads (row 3, first half) of one site
 template <typename Real, int MU, int P>
 __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const HbParams<Real>& hp, Staple18<Real>& q,
-                                          uint32_t& sweep, Real& inv_beta
+                                          uint32_t& sweep, Real& inv_beta, uint32_t hoff
 #ifdef HB_TMA
                                           ,
                                           const TmaStage<Real>* tma = nullptr
@@ -123,7 +124,8 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     SiteIdx ix;
     ix.r = (c.y + c.z + c.t + P) & 1;
     ix.h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
-    const int h = ix.h;
+    ix.ha = ix.h + (int)hoff;
+    const int h = ix.ha;
     const Nbr d = neighbours(g, c, ix.r);
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
     const uint32_t h_up = (uint32_t)(h + d.up[MU]);
@@ -200,11 +202,21 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     return ix;
 }
 
+// Hot-path kernels read the launch's expanded round keys (uniform registers); the ALT kernels key
+// Philox from two words per thread (a batched launch has one seed per replica)
+template <bool ALT>
+__device__ __forceinline__ Words philox_sel(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const RoundKeys& rk,
+                                            const RepCtx& rc)
+{
+    if (ALT) return philox4x32_10(c0, c1, c2, c3, rc.k0, rc.k1);
+    return philox_keyed(c0, c1, c2, c3, rk);
+}
+
 // rows 3 (products) to 6: staple sum, Philox, Kennedy-Pendleton, compose, store
 template <typename Real, int MU, int P, bool MEAS, bool ALT>
 __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteIdx ix, uint32_t sweep, Real inv_beta,
                                             const HbParams<Real>& hp, const m64::LogEntry* tab,
-                                            int* __restrict__ err)
+                                            const RepCtx& rc, int* __restrict__ err)
 {
     const Quat<Real>*a = q.a, *b = q.b, *cc = q.cc, *a2 = q.a2, *b2 = q.b2, *c2 = q.c2;
     const int h = ix.h, r = ix.r;
@@ -218,14 +230,14 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
             sacc.a2 += a[i].a2 + b[i].a2 + cc[i].a2 + a2[i].a2 + b2[i].a2 + c2[i].a2;
             sacc.a3 += a[i].a3 + b[i].a3 + cc[i].a3 + a2[i].a3 + b2[i].a3 + c2[i].a3;
         }
-        stq(hp.out + (uint32_t)h, sacc);
+        stq(hp.out + (uint32_t)ix.ha, sacc);
         return (Real)0;
     }
 #endif
     // [R5] counter = (s, sweep, (p<<2)|mu, n); the n = 0 draw does not depend on the links
     const uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
     const uint32_t tag = ((uint32_t)P << 2) | (uint32_t)MU;
-    const Words wd = philox_keyed(s, sweep, tag, 0u, hp.rk);
+    const Words wd = philox_sel<ALT>(s, sweep, tag, 0u, hp.rk, rc);
 
     // [R3] staple sum, nu ascending, forward then backward, products left to right;
     // the second product of every term accumulates straight into v (FMA chains).
@@ -251,7 +263,7 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
             // The rare small-alpha path: accurate library exp/log in both precisions.
             const Real E = M<Real>::exp((Real)-2 / inv_alpha);
             for (;;) {
-                const Words w = philox_keyed(s, sweep, tag, n, hp.rk);
+                const Words w = philox_sel<ALT>(s, sweep, tag, n, hp.rk, rc);
                 const Real R = M<Real>::uniform(w.w0), Rp = M<Real>::uniform(w.w1);
                 delta = -M<Real>::log(R + ((Real)1 - R) * E) * inv_alpha;
                 if (Rp * Rp <= delta * ((Real)2 - delta)) break;
@@ -264,7 +276,7 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
         } else {
             // [R6] Kennedy-Pendleton
             for (;;) {
-                const Words w = philox_keyed(s, sweep, tag, n, hp.rk);
+                const Words w = philox_sel<ALT>(s, sweep, tag, n, hp.rk, rc);
                 delta = M<Real>::kp_delta(w, inv_alpha, tab);
                 const Real Rppp = M<Real>::uniform(w.w3);
                 if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) {
@@ -291,12 +303,12 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
     }
     const Real inv = M<Real>::rsqrt(u.a0 * u.a0 + u.a1 * u.a1 + u.a2 * u.a2 + u.a3 * u.a3);
     u.a0 *= inv; u.a1 *= inv; u.a2 *= inv; u.a3 *= inv;
-    stq(hp.out + (uint32_t)h, u);
+    stq(hp.out + (uint32_t)ix.ha, u);
     return MEAS ? u.a0 * w.a0 - u.a1 * w.a1 - u.a2 * w.a2 - u.a3 * w.a3 : (Real)0;  // 1/2 Tr(U' w)
 }
 
 template <typename Real, int MU, int P, bool MEAS, bool ALT>
-__device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp,
+__device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp, uint32_t rep,
                                               int* __restrict__ err
 #ifdef HB_TMA
                                               ,
@@ -309,12 +321,20 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     uint32_t sweep;
     Real inv_beta;
     Staple18<Real> q;
+    RepCtx rc = {0u, 0u, hp.rk.k[0], hp.rk.k[1]};
+    if (ALT) rc = {rep, rep * hp.rep_stride, hp.rk.k[0], hp.rk.k[1]};
 #ifdef HB_TMA
-    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, tma);
+    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, rc.hoff, tma);
 #else
-    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta);
+    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, rc.hoff);
 #endif
-    return update_link<Real, MU, P, MEAS, ALT>(q, ix, sweep, inv_beta, hp, kLogTab, err);
+    if (ALT && hp.reps) {  // batched launch: this replica's coupling and seed
+        const RepParams rp = hp.reps[rep];
+        inv_beta = (Real)rp.inv_beta;
+        rc.k0 = (uint32_t)rp.seed;
+        rc.k1 = (uint32_t)(rp.seed >> 32);
+    }
+    return update_link<Real, MU, P, MEAS, ALT>(q, ix, sweep, inv_beta, hp, kLogTab, rc, err);
 }
 
 // Resident CTAs per SM that ptxas must allow: this is the register budget that lets it
@@ -340,7 +360,12 @@ template <typename Real, int MU, int P, bool MEAS, bool ALT, int LHX, int LY, in
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::value)
     heatbath_tiled_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
-    const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z);
+    uint32_t rep = 0, bzt = blockIdx.z;
+    if (ALT && hp.reps) {  // batched launch: grid z = (replica, z-t tile)
+        rep = bzt / hp.nzt;
+        bzt -= rep * hp.nzt;
+    }
+    const Site c = tile_site<LHX, LY, LZ, LT>(g, bzt);
 #ifdef HB_TMA
     __shared__ __align__(128) typename LinkPtr<Real>::type stage_buf[kTmaSlots << (LHX + LY + LZ + LT)];
     __shared__ __align__(8) uint64_t stage_bar;
@@ -350,14 +375,15 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::va
     }
     __syncthreads();  // ahead of griddepcontrol.wait: overlaps the predecessor's tail
     const TmaStage<Real> tma = {stage_buf, &stage_bar, 1 << LHX};
-    const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, err, &tma);
+    const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err, &tma);
 #else
-    const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, err);
+    const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err);
 #endif
     if (MEAS) {  // one fp64 partial per CTA, fixed order
         __shared__ double red[kBlock / 32];
         const double tot = block_sum_end(e, red);
-        if (threadIdx.x == 0) hp.epart[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = tot;
+        if (threadIdx.x == 0)
+            hp.epart[(size_t)rep * hp.epart_stride + blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * bzt)] = tot;
     }
 }
 
@@ -376,12 +402,12 @@ __global__ void __launch_bounds__(kBlock)
         c.y = (int)(q - q2 * (uint32_t)g.n[1]);
         c.t = (int)(q2 / (uint32_t)g.n[2]);
         c.z = (int)(q2 - (uint32_t)c.t * (uint32_t)g.n[2]);
-        e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, err);
+        e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, blockIdx.y, err);  // grid y = replica
     }
     if (MEAS) {
         __shared__ double red[kBlock / 32];
         const double tot = block_sum_end(e, red);
-        if (threadIdx.x == 0) hp.epart[blockIdx.x] = tot;
+        if (threadIdx.x == 0) hp.epart[(size_t)blockIdx.y * hp.epart_stride + blockIdx.x] = tot;
     }
 }
 
@@ -435,8 +461,8 @@ void choose_tiling(Geom& g)
 
 template <typename Real, int MU, int P, bool MEAS, bool ALT>
 static int launch_substep_t(void* links, const Geom& g, double beta, double creutz_below, uint64_t seed,
-                            uint32_t sweep, int* err, double* epart, const RunState* state, bool overlap,
-                            cudaStream_t st)
+                            uint32_t sweep, int* err, double* epart, const RunState* state, const RepParams* reps,
+                            int nrep, bool overlap, cudaStream_t st)
 {
     typedef typename LinkPtr<Real>::type L;
     HbParams<Real> hp;
@@ -451,7 +477,11 @@ static int launch_substep_t(void* links, const Geom& g, double beta, double creu
     hp.out = (L*)links + (size_t)(P * 4 + MU) * g.vh;
     hp.epart = epart;
     hp.state = state;
-    const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
+    hp.reps = reps;
+    hp.rep_stride = 8u * g.vh;
+    hp.nzt = (uint32_t)(g.nb[2] * g.nb[3]);
+    hp.epart_stride = (uint32_t)(3 * heatbath_ctas(g));
+    const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3] * nrep));
     if (g.tile == 0) {
         launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>,
                   grid, dim3(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3])), st, overlap, g, hp,
@@ -461,8 +491,8 @@ static int launch_substep_t(void* links, const Geom& g, double beta, double creu
                   grid, dim3(1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3])), st, overlap, g, hp,
                   err);
     } else {
-        launch_ex(heatbath_linear_kernel<Real, MU, P, MEAS, ALT>, dim3((unsigned)heatbath_ctas(g)), dim3(kBlock), st,
-                  overlap, g, hp, err);
+        launch_ex(heatbath_linear_kernel<Real, MU, P, MEAS, ALT>, dim3((unsigned)heatbath_ctas(g), (unsigned)nrep),
+                  dim3(kBlock), st, overlap, g, hp, err);
     }
     return 1;
 }
@@ -476,11 +506,12 @@ size_t heatbath_ctas(const Geom& g)
 
 template <typename Real, bool ALT>
 static int launch_substep_p(void* links, const Geom& g, int mu, int parity, double beta, double cb, uint64_t seed,
-                            uint32_t sweep, int* err, double* epart, const RunState* state, bool overlap,
-                            cudaStream_t st)
+                            uint32_t sweep, int* err, double* epart, const RunState* state, const RepParams* reps,
+                            int nrep, bool overlap, cudaStream_t st)
 {
-#define SU2_HB(MU_, P_, MEAS_, EP_) \
-    return launch_substep_t<Real, MU_, P_, MEAS_, ALT>(links, g, beta, cb, seed, sweep, err, EP_, state, overlap, st)
+#define SU2_HB(MU_, P_, MEAS_, EP_)                                                                               \
+    return launch_substep_t<Real, MU_, P_, MEAS_, ALT>(links, g, beta, cb, seed, sweep, err, EP_, state, reps, nrep, \
+                                                       overlap, st)
     if (epart && parity == 1 && mu >= 1) {  // the three measuring kernels
         switch (mu) {
             case 1: SU2_HB(1, 1, true, epart);
@@ -507,13 +538,18 @@ static int launch_substep_p(void* links, const Geom& g, int mu, int parity, doub
 // partials; ignored by the other sub-steps.
 // `creutz_below` [R15]: 0 = Kennedy-Pendleton everywhere (the hot-path kernels); otherwise the ALT
 // kernels, which use Creutz's draw on links with alpha < creutz_below (+inf = on every link).
+// `reps` (nullable, [device]): batched launch over `nrep` configurations stored one after the other
+// from `links`, each with its own 1/beta and seed (beta and seed arguments are then unused); `epart`
+// then holds nrep * 3 * heatbath_ctas(g) partials, replica-major. Batched launches use the ALT kernels.
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
                             double creutz_below, uint64_t seed, uint32_t sweep, int* err, double* epart,
-                            const RunState* state, bool overlap, cudaStream_t st)
+                            const RunState* state, bool overlap, cudaStream_t st, const RepParams* reps, int nrep)
 {
-    const bool alt = creutz_below > 0.0;
-#define SU2_HB(REAL_, ALT_) \
-    launch_substep_p<REAL_, ALT_>(links, g, mu, parity, beta, creutz_below, seed, sweep, err, epart, state, overlap, st)
+    const bool alt = creutz_below > 0.0 || reps != nullptr;
+    if (!reps) nrep = 1;
+#define SU2_HB(REAL_, ALT_)                                                                                      \
+    launch_substep_p<REAL_, ALT_>(links, g, mu, parity, beta, creutz_below, seed, sweep, err, epart, state, reps, \
+                                  nrep, overlap, st)
     if (precision == 32) return alt ? SU2_HB(float, true) : SU2_HB(float, false);
     return alt ? SU2_HB(double, true) : SU2_HB(double, false);
 #undef SU2_HB

@@ -49,8 +49,9 @@ struct Scratch {
     double* out;        // [device] 2 + kMaxR doubles: plaquette, polyakov, correlator
     int* err;           // [device] sticky error flags (bit 0: KP trial cap hit)
     RunState* state;    // [device] loop state of su2_run
-    double* slots;      // [device] step tail: 2 doubles per CTA of the Polyakov kernel (<= V/Nt/64 + 1 CTAs)
-    unsigned* ticket;   // [device] step tail: arrival counter, zero between steps
+    double* slots;      // [device] step tail: 2 doubles per CTA of the Polyakov kernel (<= V/Nt/64 + 1 CTAs), per replica
+    unsigned* ticket;   // [device] step tail: arrival counters (one per replica), zero between steps
+    RepParams* reps;    // [device] batch: per-replica 1/beta and seed
 };
 constexpr int kMaxR = 128;
 
@@ -62,7 +63,8 @@ size_t partials_needed(const Geom& g);
 int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st);
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
                             double creutz_below, uint64_t seed, uint32_t sweep, int* err, double* epart,
-                            const RunState* state, bool overlap, cudaStream_t st);
+                            const RunState* state, bool overlap, cudaStream_t st, const RepParams* reps = nullptr,
+                            int nrep = 1);
 size_t heatbath_ctas(const Geom& g);
 int launch_final_sum(const double* partials, size_t n, double scale, double* dev_dst, cudaStream_t st);
 int launch_set_run_state(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index,
@@ -72,7 +74,7 @@ int launch_polyakov_partials(const void* links, const Geom& g, int precision, co
                              cudaStream_t st);
 int launch_polyakov_step(const void* links, const Geom& g, int precision, const Scratch& sc, const double* epart,
                          size_t n_epart, double scale_plaq, double* dev_dst, RunState* state, bool overlap,
-                         cudaStream_t st);
+                         cudaStream_t st, int nrep = 1);
 int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
                      cudaStream_t st);
 int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,

@@ -132,41 +132,44 @@ struct StepTail {
     const double* epart;  // [device] fused-plaquette partials of the sweep; NULL = no tail (plain Polyakov kernel)
     size_t n_epart;
     double scale_plaq, scale_poly;
-    double* slots;        // [device] 2 * gridDim.x doubles
-    unsigned* ticket;     // [device] zero between steps
-    double* dst;          // [device] 2 doubles (ignored when state != NULL)
+    double* slots;        // [device] 2 * gridDim.x doubles per replica
+    unsigned* ticket;     // [device] one per replica, zero between steps
+    double* dst;          // [device] 2 doubles per replica (ignored when state != NULL)
     RunState* state;      // su2_run: destination state->out[2*index..], then sweep and index advance
 };
 __device__ __forceinline__ void step_tail(const StepTail& tl, double poly_tot, double* red)
 {
     __shared__ bool is_last;
-    const unsigned G = gridDim.x, b = blockIdx.x;
+    const unsigned G = gridDim.x, b = blockIdx.x, rep = blockIdx.y;  // grid y = replica of a batched launch
+    const double* epart = tl.epart + (size_t)rep * tl.n_epart;
+    double* slots = tl.slots + (size_t)rep * 2 * G;
+    unsigned* ticket = tl.ticket + rep;
     const size_t chunk = (tl.n_epart + G - 1) / G;
     const size_t lo = (size_t)b * chunk, hi = (lo + chunk < tl.n_epart) ? lo + chunk : tl.n_epart;
     double acc = 0.0;
-    for (size_t i = lo + threadIdx.x; i < hi; i += blockDim.x) acc += __ldcg(tl.epart + i);
+    for (size_t i = lo + threadIdx.x; i < hi; i += blockDim.x) acc += __ldcg(epart + i);
     const double ea = block_sum(acc, red);
     if (threadIdx.x == 0) {
-        tl.slots[2 * b] = ea;
-        tl.slots[2 * b + 1] = poly_tot;
+        slots[2 * b] = ea;
+        slots[2 * b + 1] = poly_tot;
         __threadfence();
-        is_last = atomicAdd(tl.ticket, 1u) == G - 1;
+        is_last = atomicAdd(ticket, 1u) == G - 1;
     }
     __syncthreads();
     if (!is_last) return;
     __threadfence();
     double sa = 0.0, sb = 0.0;
     for (unsigned i = threadIdx.x; i < G; i += blockDim.x) {
-        sa += __ldcg(tl.slots + 2 * i);
-        sb += __ldcg(tl.slots + 2 * i + 1);
+        sa += __ldcg(slots + 2 * i);
+        sb += __ldcg(slots + 2 * i + 1);
     }
     const double ta = block_sum(sa, red);
     const double tb = block_sum(sb, red);
     if (threadIdx.x == 0) {
-        double* dst = tl.state ? tl.state->out + 2 * (size_t)tl.state->index : tl.dst;
+        double* dst = tl.state ? tl.state->out + 2 * (size_t)tl.state->index : tl.dst + 2 * (size_t)rep;
         dst[0] = ta * tl.scale_plaq;
         dst[1] = tb * tl.scale_poly;
-        *tl.ticket = 0u;
+        *ticket = 0u;
     }
     if (tl.state)  // su2_run: advance every copy of the loop state (this CTA is the last one running)
         for (int i = threadIdx.x; i < kRunCopies; i += blockDim.x) {
@@ -190,6 +193,8 @@ __global__ void __launch_bounds__(kBlock)
     // every thread waits (the tail reads that kernel's partials), links are read through L2
     grid_dep_wait();
     grid_dep_launch();
+    links += (size_t)blockIdx.y * 8 * g.vh;  // grid y = replica of a batched launch (else 0)
+    if (field) field += (size_t)blockIdx.y * v3;
     double val = 0.0;
     if (s3 < v3) {
         const uint32_t x = s3 % (uint32_t)g.n[0];
@@ -234,6 +239,8 @@ __global__ void __launch_bounds__(kBlock)
     const int len = g.n[3] / S, t0 = seg * len;
     grid_dep_wait();
     grid_dep_launch();
+    links += (size_t)blockIdx.y * 8 * g.vh;  // grid y = replica of a batched launch (else 0)
+    if (field) field += (size_t)blockIdx.y * v3;
     if (s3 < v3) {
         const uint32_t x = s3 % (uint32_t)g.n[0];
         const uint32_t q = s3 / (uint32_t)g.n[0];
@@ -400,7 +407,7 @@ int launch_final_sum(const double* partials, size_t n, double scale, double* dev
 
 template <typename Real>
 static unsigned launch_polyakov_t(const void* links, const Geom& g, const Scratch& sc, const StepTail& tl,
-                                  bool overlap, cudaStream_t st)
+                                  bool overlap, cudaStream_t st, int nrep = 1)
 {
     typedef typename LinkPtr<Real>::type L;
     const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
@@ -409,18 +416,18 @@ static unsigned launch_polyakov_t(const void* links, const Geom& g, const Scratc
     const bool small = v3 < 148ull * 1024ull;
     if (small && nt >= 16 && nt % 4 == 0) {
         const unsigned grid = (unsigned)((v3 + kBlock / 4 - 1) / (kBlock / 4));
-        launch_ex(polyakov_split_kernel<Real, 4>, dim3(grid), dim3(kBlock), st, overlap, (const L*)links, g, sc.field,
+        launch_ex(polyakov_split_kernel<Real, 4>, dim3(grid, (unsigned)nrep), dim3(kBlock), st, overlap, (const L*)links, g, sc.field,
                   sc.partials, tl);
         return grid;
     }
     if (small && nt >= 8 && nt % 2 == 0) {
         const unsigned grid = (unsigned)((v3 + kBlock / 2 - 1) / (kBlock / 2));
-        launch_ex(polyakov_split_kernel<Real, 2>, dim3(grid), dim3(kBlock), st, overlap, (const L*)links, g, sc.field,
+        launch_ex(polyakov_split_kernel<Real, 2>, dim3(grid, (unsigned)nrep), dim3(kBlock), st, overlap, (const L*)links, g, sc.field,
                   sc.partials, tl);
         return grid;
     }
     const unsigned grid = blocks_for(v3);
-    launch_ex(polyakov_kernel<Real>, dim3(grid), dim3(kBlock), st, overlap, (const L*)links, g, sc.field, sc.partials,
+    launch_ex(polyakov_kernel<Real>, dim3(grid, (unsigned)nrep), dim3(kBlock), st, overlap, (const L*)links, g, sc.field, sc.partials,
               tl);
     return grid;
 }
@@ -437,14 +444,14 @@ int launch_polyakov_partials(const void* links, const Geom& g, int precision, co
 // the last kernel of a step: Polyakov loop + both final sums (see step_tail)
 int launch_polyakov_step(const void* links, const Geom& g, int precision, const Scratch& sc, const double* epart,
                          size_t n_epart, double scale_plaq, double* dev_dst, RunState* state, bool overlap,
-                         cudaStream_t st)
+                         cudaStream_t st, int nrep)
 {
     const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
     const StepTail tl = {epart, n_epart, scale_plaq, 1.0 / (double)v3, sc.slots, sc.ticket, dev_dst, state};
     if (precision == 32)
-        launch_polyakov_t<float>(links, g, sc, tl, overlap, st);
+        launch_polyakov_t<float>(links, g, sc, tl, overlap, st, nrep);
     else
-        launch_polyakov_t<double>(links, g, sc, tl, overlap, st);
+        launch_polyakov_t<double>(links, g, sc, tl, overlap, st, nrep);
     return 1;
 }
 

@@ -504,3 +504,80 @@ def test_run_follows_set_draw_and_bad_method_is_rejected(pkg):
     with pytest.raises(pkg.SU2Error):
         pkg.su2_set_draw(a.h, 7)
     a.close(); b.close()
+
+
+# ---------------------------------------------------------------- replica batches (S8(f) NEXT-2)
+@pytest.mark.parametrize("method", ["kp", "auto"])
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", [(16, 16, 16, 4), (32, 4, 4, 2), (8, 8, 8, 8), (6, 4, 10, 2)])
+def test_batch_equals_single_lattices_bitwise_and_matches_oracle(pkg, oracle_draw, dims, prec, method):
+    """A batch of 5 replicas (config 2's beta scan: own beta, own seed each) stepped by
+    su2_batch_sweep_measure equals, bit for bit, 5 single-lattice handles stepped by
+    su2_heatbath_sweep_measure (same Philox streams, same arithmetic, same reduction order);
+    and replica 3 after one teacher-forced batch step matches the oracle."""
+    import torch
+    betas = [2.2, 2.3, 2.4, 2.5, 0.6 if method == "auto" else 2.6]
+    seeds = [100 + i for i in range(5)]
+    R, n = 5, 3
+    bat = pkg.Lattice(dims, prec, replicas=R)
+    bat.set_draw(method)
+    bat.batch_init("hot", seeds)
+    ob = torch.zeros(2 * R * n, dtype=torch.float64, device="cuda")
+    for i in range(n):
+        bat.batch_sweep_measure(betas, i, ob, i)
+    torch.cuda.synchronize()
+    ob = ob.cpu().numpy().reshape(n, R, 2)
+    for r in range(R):
+        one = pkg.Lattice(dims, prec)
+        one.set_draw(method)
+        one.init("hot", seeds[r])
+        o1 = torch.zeros(2 * n, dtype=torch.float64, device="cuda")
+        for i in range(n):
+            one.sweep_measure(betas[r], i, o1, i)
+        torch.cuda.synchronize()
+        bat.select(r)
+        assert (bat.get_links() == one.get_links()).all(), r
+        assert (ob[:, r, :] == o1.cpu().numpy().reshape(n, 2)).all(), r
+        # single-lattice calls act on the selected replica
+        assert bat.mean_plaquette() == one.mean_plaquette()
+        one.close()
+    # teacher-forced against the oracle: load a known configuration into replica 3 only
+    mode = MODE[prec]
+    oracle_draw(method)
+    # (a near-ordered configuration, as in test_sweep_on_smooth_lattice_matches_oracle: over a whole fp32
+    # sweep of a Haar-random lattice a rare link with a tiny staple norm amplifies the rounding of its
+    # neighbours past 1e-5; the sub-step tests cover random lattices)
+    L = workloads.smooth_links(dims, 77, 0.3, oracle.dtype(mode))
+    bat.select(3)
+    bat.set_links(L)
+    bat.batch_sweep_measure(betas, 9, torch.zeros(2 * R, dtype=torch.float64, device="cuda"), 0)
+    g = bat.get_links()
+    V = oracle.volume(dims)
+    mg = np.ones((V, 4))
+    oracle.heatbath_sweep(dims, L, betas[3], seeds[3], 9, mode, margin=mg)
+    flips = assert_links_match(g, L, prec, mg, max_flips=3, what="batch replica 3")
+    if flips == 0:
+        assert abs(bat.mean_plaquette() - oracle.mean_plaquette(dims, L, mode)) < PTOL[prec]
+    bat.close()
+
+
+def test_batch_argument_checks(pkg):
+    import torch
+    with pytest.raises(pkg.SU2Error):
+        pkg.su2_lattice_create_batch(8, 8, 8, 8, 32, 0)
+    bat = pkg.Lattice((8, 8, 8, 4), 32, replicas=2)
+    assert pkg.su2_replicas(bat.h) == 2
+    out = torch.zeros(4, dtype=torch.float64, device="cuda")
+    with pytest.raises(pkg.SU2Error):     # not initialised
+        bat.batch_sweep_measure([2.3, 2.3], 0, out, 0)
+    bat.init("hot", 1)                    # replica 0 only
+    with pytest.raises(pkg.SU2Error):
+        bat.batch_sweep_measure([2.3, 2.3], 0, out, 0)
+    bat.select(1)
+    bat.init("cold", 2)
+    bat.batch_sweep_measure([2.3, 2.3], 0, out, 0)
+    with pytest.raises(pkg.SU2Error):
+        bat.batch_sweep_measure([2.3, -1.0], 1, out, 0)
+    with pytest.raises(pkg.SU2Error):
+        bat.select(2)
+    bat.close()
