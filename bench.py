@@ -257,6 +257,25 @@ def time_aux(pkg, torch, workloads):
             rec["correlator_r1"] = float(c[0])
         out[name] = rec
         lat.close()
+    # replica batches (S8(f) NEXT-2): config 2's beta scan, R lattices stepped by the launches of one
+    w = workloads.BY_NAME["C2_16^3x4"]
+    for R in (5, 20):
+        bat = pkg.Lattice(w.dims, 32, replicas=R)
+        bat.batch_init(w.start, [w.seed + r for r in range(R)])
+        betas = [2.2 + 0.1 * (r % 5) for r in range(R)]
+        n = 200
+        obs = torch.zeros(2 * R * n, dtype=torch.float64, device=bat.device)
+        for i in range(10):
+            bat.batch_sweep_measure(betas, i, obs, i)
+        bat.synchronize()
+        t0 = time.perf_counter()
+        for i in range(n):
+            bat.batch_sweep_measure(betas, 10 + i, obs, i)
+        bat.synchronize()
+        dt = time.perf_counter() - t0
+        out[f"C2_16^3x4_batch{R}"] = {"us_per_round": dt / n * 1e6, "value": R * w.links * n / dt, "unit": UNIT,
+                                      "replicas": R, "precision": 32, "rounds": n}
+        bat.close()
     return out
 
 
