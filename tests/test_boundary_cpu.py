@@ -57,6 +57,15 @@ def test_argument_validation_without_gpu(built):
     assert L.su2_lattice_create(7, 8, 8, 8, 64, C.byref(h)) == pkg.SU2_EARG and not h.value
     assert L.su2_lattice_create(8, 8, 8, 8, 64, None) == pkg.SU2_EARG
     assert L.su2_lattice_destroy(None) == pkg.SU2_OK
+    # batches: replica count, 32-bit link index over the whole batch, replica in the grid
+    assert L.su2_lattice_create_batch(8, 8, 8, 8, 64, 0, C.byref(h)) == pkg.SU2_EARG and not h.value
+    assert L.su2_lattice_create_batch(8, 8, 8, 8, 64, 70000, C.byref(h)) == pkg.SU2_EARG
+    assert L.su2_lattice_create_batch(64, 64, 64, 64, 32, 64, C.byref(h)) == pkg.SU2_EARG  # 64 * 4V = 2^32
+    assert L.su2_replicas(None) == 0
+    assert L.su2_select_replica(None, 0) == pkg.SU2_EARG
+    assert L.su2_batch_init(None, 0, None) == pkg.SU2_EARG
+    assert L.su2_batch_sweep_measure(None, None, 0, None, 0) == pkg.SU2_EARG
+    assert L.su2_set_draw(None, 0) == pkg.SU2_EARG
     assert L.su2_init(None, 0, 1) == pkg.SU2_EARG
     assert L.su2_heatbath_sweep(None, 2.3, 0) == pkg.SU2_EARG
     assert L.su2_strerror(pkg.SU2_ESTATE).decode().startswith("bad state")
