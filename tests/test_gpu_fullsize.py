@@ -71,3 +71,45 @@ def test_sampled_link_parity_at_bench_sizes(dims, prec, start, beta):
         del after
     assert flips <= (0 if prec == 64 else 2)
     lat.close()
+
+
+@pytest.mark.parametrize("prec", [32, 64])
+def test_sampled_link_parity_at_32c4_with_auto_draw(prec):
+    """The ALT kernels (draw selection [R15]) at a bench size: 32^4, beta = 0.5 from a hot start, where
+    'auto' takes Creutz's draw on most links and KP on the rest; sampled sites recomputed by the oracle."""
+    import paper_1104_5432_b200 as pkg
+    dims, beta, seed, mode = (32, 32, 32, 32), 0.5, 7, MODE[prec]
+    for m in ("f64", "f32"):
+        oracle.set_draw("auto", m)
+    try:
+        lat = pkg.Lattice(dims, prec)
+        lat.set_draw("auto")
+        lat.init("hot", seed)
+        lat.sweep(beta, 0)
+        before = lat.get_links()
+        V = oracle.volume(dims)
+        rng = np.random.default_rng(9)
+        par_of = lambda s: (s % 32 + s // 32 % 32 + s // 1024 % 32 + s // 32768) % 2
+        flips = n_creutz = n_kp = 0
+        for mu, p in ((0, 1), (3, 0)):
+            lat.set_links(before)
+            lat.substep(beta, 1, mu, p)
+            after = lat.get_links()
+            cand = np.concatenate([rng.integers(0, V, size=1200), [0, V - 1, 31, V - 32]])
+            cand = np.unique(cand[par_of(cand) == p])[:400]
+            for s in cand:
+                u, tr, mg = oracle.heatbath_link(dims, before, beta, seed, 1, int(s), mu, mode)
+                k = np.linalg.norm(oracle.staple(dims, before, int(s), mu, mode).astype(np.float64))
+                n_creutz += beta * k < oracle.ALPHA_C
+                n_kp += beta * k >= oracle.ALPHA_C
+                d = np.abs(after[s, mu].astype(np.float64) - u.astype(np.float64)).max()
+                if d > TOL[prec]:
+                    assert mg < FLIP[prec], (s, mu, d, mg)
+                    flips += 1
+            del after
+        assert n_creutz > 100 and n_kp > 20      # both branches sampled
+        assert flips <= (0 if prec == 64 else 3)
+        lat.close()
+    finally:
+        for m in ("f64", "f32", "f32x"):
+            oracle.set_draw("kp", m)
