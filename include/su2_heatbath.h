@@ -209,6 +209,68 @@ SU2_API int su2_set_links(su2_lattice* lat, const void* host_src, size_t bytes);
 /* Block until all work enqueued on the handle's stream has finished. */
 SU2_API int su2_synchronize(su2_lattice* lat);
 
+/* ---------------------------------------------------------------------------------------
+ * S8(f) NEXT-4: the lattice split into time slabs, one per GPU — the paper's second mode
+ * ("2 GPUs ... OpenMP"; the exchange itself is not described there;
+ * SURVEY.md §8(e) states it; DESIGN.md §6.9 is the design). Not part of the benchmarked path.
+ *
+ * A slab owns the Lt global time slices t0 .. t0+Lt-1 (t0, Lt even, Lt >= 2) of an
+ * Nx x Ny x Nz x Nt lattice and stores Lt + 4 local slices: local slice t is a copy of global
+ * slice (t0 - 2 + t) mod Nt; slices 2 .. Lt+1 are the interior (updated here), slices 1 and Lt+2
+ * are the halos the staples read (owned by the slab below / above), slices 0 and Lt+3 are
+ * padding that keeps local and global site parity equal. The handle is an ordinary lattice of
+ * local extents Nx x Ny x Nz x (Lt+4) as far as memory goes: same device layout with V = local
+ * sites, and su2_get_links / su2_set_links move the Lt+4 local slices in canonical order.
+ *
+ * One sub-step (mu, parity) of the whole lattice = su2_slab_substep on every slab, in any order or
+ * concurrently, then a barrier: the kernel that updates a slab's first / last interior slice also
+ * stores those links into the halo of the slab below / above (plain stores into peer memory over
+ * NVLink, or into another buffer of the same device), so there is no separate exchange step, and
+ * within a sub-step no slab reads what another one writes. Draws are keyed by the GLOBAL site [R5]:
+ * the result is the one su2_heatbath_substep gives on the unsplit lattice, bit for bit.
+ * The whole-lattice calls (su2_heatbath_sweep, su2_heatbath_sweep_measure, su2_run, su2_measure*,
+ * su2_polyakov_correlator, su2_batch_*) return SU2_ESTATE on a slab handle; su2_init (every local
+ * slice, halos included, from its global site), su2_set_seed, su2_set_draw, su2_set_stream,
+ * su2_heatbath_substep (= su2_slab_substep without the fused plaquette), su2_get/set_links work. */
+SU2_API size_t su2_slab_bytes(int Nx, int Ny, int Nz, int Lt, int precision); /* 0 = invalid */
+SU2_API int su2_slab_create(int Nx, int Ny, int Nz, int Nt, int precision, int t0, int Lt, su2_lattice** out);
+SU2_API int su2_slab_create_external(int Nx, int Ny, int Nz, int Nt, int precision, int t0, int Lt, void* dev_links,
+                                     size_t bytes, void* cuda_stream, su2_lattice** out);
+
+/* Where the edge slices are also stored: lo_links / hi_links [device, this or a peer device] = the
+ * link buffers (su2_device_links) of the slabs that own global slices t0-1 and t0+Lt (periodic; with
+ * two slabs both are the other slab, with one slab both are the handle's own buffer), lo_Lt / hi_Lt
+ * their interior extents. The buffers must stay valid while sub-steps run. Errors: SU2_EARG, SU2_ESTATE. */
+SU2_API int su2_slab_set_peers(su2_lattice* lat, void* lo_links, int lo_Lt, void* hi_links, int hi_Lt);
+
+/* Rows 2-6 on the interior slices + the stores into the neighbours' halos. fuse_plaquette != 0: the
+ * sub-steps (mu >= 1, parity 1) also keep the plaquette partials of their planes.
+ * Asynchronous. The caller provides the barrier between sub-steps (stream order on one device; a
+ * stream-ordered collective or an event across devices). */
+SU2_API int su2_slab_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, int mu, int parity, int fuse_plaquette);
+
+/* Row 7 on a slab: *dev_out [device] = (sum over the plaquettes based at interior sites) / (6 V_global),
+ * so the values of all slabs add up to the mean plaquette [R10]. fused != 0: from the partials of
+ * the last sweep's fused sub-steps; else by the plaquette kernel (needs a current upper halo).
+ * Asynchronous. */
+SU2_API int su2_slab_plaquette(su2_lattice* lat, int fused, double* dev_out);
+
+/* Row 8 across slabs [R11]: the ordered product of the time links continues from slab to slab.
+ *   dev_prev [device] NxNyNz links (the product over all slices below t0, per spatial site, index
+ *            x + Nx (y + Ny z)), NULL exactly on the slab with t0 = 0;
+ *   dev_next [device, nullable] receives the product including this slab's slices;
+ *   dev_out  [device, nullable] receives the spatial mean of 1/2 Tr of that product (the Polyakov
+ *            loop when this is the last slab).
+ * Same left-to-right association as the single-lattice loop. Asynchronous. */
+SU2_API int su2_slab_polyakov(su2_lattice* lat, const void* dev_prev, void* dev_next, double* dev_out);
+
+/* CUDA IPC plumbing for one process per GPU: export the (library-allocated: su2_slab_create) link
+ * buffer as a 64-byte handle [host]; open / close such a handle in another process. su2_ipc_open
+ * returns a [device] pointer valid in the calling process for su2_slab_set_peers. */
+SU2_API int su2_ipc_export(su2_lattice* lat, void* handle64);
+SU2_API int su2_ipc_open(const void* handle64, void** dev_ptr);
+SU2_API int su2_ipc_close(void* dev_ptr);
+
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 SU2_API uint64_t su2_launch_count(const su2_lattice* lat);
 

@@ -54,6 +54,16 @@ _SIGNATURES = {
     "su2_get_links": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "su2_set_links": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "su2_synchronize": (C.c_int, [C.c_void_p]),
+    "su2_slab_bytes": (C.c_size_t, [C.c_int] * 5),
+    "su2_slab_create": (C.c_int, [C.c_int] * 7 + [C.POINTER(C.c_void_p)]),
+    "su2_slab_create_external": (C.c_int, [C.c_int] * 7 + [C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]),
+    "su2_slab_set_peers": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int]),
+    "su2_slab_substep": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32, C.c_int, C.c_int, C.c_int]),
+    "su2_slab_plaquette": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "su2_slab_polyakov": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "su2_ipc_export": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "su2_ipc_open": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p)]),
+    "su2_ipc_close": (C.c_int, [C.c_void_p]),
     "su2_launch_count": (C.c_uint64, [C.c_void_p]),
     "su2_device_links": (C.c_void_p, [C.c_void_p]),
     "su2_last_error": (C.c_char_p, [C.c_void_p]),
@@ -224,6 +234,62 @@ def su2_synchronize(h):
 
 def su2_launch_count(h):
     return lib().su2_launch_count(h)
+
+
+# ---- time slabs (S8(f) NEXT-4; drivers in paper_1104_5432_b200.slabs) --------------------------
+def su2_slab_bytes(Nx, Ny, Nz, Lt, precision):
+    return lib().su2_slab_bytes(Nx, Ny, Nz, Lt, precision)
+
+
+def su2_slab_create(Nx, Ny, Nz, Nt, precision, t0, Lt):
+    h = C.c_void_p()
+    _check(lib().su2_slab_create(Nx, Ny, Nz, Nt, precision, t0, Lt, C.byref(h)))
+    return h
+
+
+def su2_slab_create_external(Nx, Ny, Nz, Nt, precision, t0, Lt, dev_ptr, nbytes, cuda_stream=0):
+    h = C.c_void_p()
+    _check(lib().su2_slab_create_external(Nx, Ny, Nz, Nt, precision, t0, Lt, C.c_void_p(dev_ptr), nbytes,
+                                          C.c_void_p(cuda_stream), C.byref(h)))
+    return h
+
+
+def su2_slab_set_peers(h, lo_ptr, lo_Lt, hi_ptr, hi_Lt):
+    _check(lib().su2_slab_set_peers(h, C.c_void_p(lo_ptr), lo_Lt, C.c_void_p(hi_ptr), hi_Lt), h)
+
+
+def su2_slab_substep(h, beta, sweep_idx, mu, parity, fuse_plaquette=0):
+    _check(lib().su2_slab_substep(h, beta, sweep_idx, mu, parity, int(fuse_plaquette)), h)
+
+
+def su2_slab_plaquette(h, fused, dev_out_ptr):
+    _check(lib().su2_slab_plaquette(h, int(fused), C.c_void_p(dev_out_ptr)), h)
+
+
+def su2_slab_polyakov(h, dev_prev_ptr, dev_next_ptr, dev_out_ptr):
+    _check(lib().su2_slab_polyakov(h, C.c_void_p(dev_prev_ptr or None), C.c_void_p(dev_next_ptr or None),
+                                   C.c_void_p(dev_out_ptr or None)), h)
+
+
+def su2_ipc_export(h):
+    buf = C.create_string_buffer(64)
+    _check(lib().su2_ipc_export(h, buf), h)
+    return buf.raw
+
+
+def su2_ipc_open(handle64):
+    assert len(handle64) == 64
+    p = C.c_void_p()
+    _check(lib().su2_ipc_open(C.c_char_p(handle64), C.byref(p)))
+    return p.value
+
+
+def su2_ipc_close(dev_ptr):
+    _check(lib().su2_ipc_close(C.c_void_p(dev_ptr)))
+
+
+def su2_device_links(h):
+    return lib().su2_device_links(h)
 
 
 # ---- convenience wrapper ---------------------------------------------------------------

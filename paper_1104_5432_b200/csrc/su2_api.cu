@@ -39,6 +39,11 @@ struct su2_lattice {
     uint64_t* rep_seed;        // [host] nrep
     unsigned char* rep_init;   // [host] nrep
     RepParams* rep_host;       // [host] nrep: what sc.reps holds
+    // time slab of a lattice split over GPUs: local slices = 2 halo + Lt interior + 2 halo
+    bool slab;
+    int nt_glob, t0, Lt;     // global time extent, first global slice of the interior, interior slices
+    SlabCtx sctx;            // peers (set by su2_slab_set_peers)
+    bool peers_set;
     void* stage;       // canonical-order staging buffer of su2_get_links / su2_set_links (lazy, kept)
     int sticky;  // sticky error code
     char msg[256];
@@ -65,6 +70,11 @@ static int fail(su2_lattice* lat, int code, const char* what, cudaError_t ce = c
         if (!(lat)) return SU2_EARG;     \
         if ((lat)->sticky) return (lat)->sticky; \
     } while (0)
+// calls that step or measure a whole lattice by themselves: a slab needs its neighbours between sub-steps
+#define NOT_ON_A_SLAB(lat, what)                                                                    \
+    do {                                                                                            \
+        if ((lat)->slab) return fail(lat, SU2_ESTATE, what ": not available on a slab handle (su2_slab_*)"); \
+    } while (0)
 // last_substep value after the Polyakov kernel of a step: sub-step (0,0) may overlap its tail
 // (it waits for it like for a predecessor sub-step; that kernel itself waited for (3,1))
 static const int kAfterStepTail = 8;
@@ -83,7 +93,7 @@ static void enqueue_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, i
     if (!state) st = lat->stream;
     lat->launches += launch_heatbath_substep(lat->links, lat->g, lat->precision, mu, parity, beta,
                                              lat->creutz_below, lat->seed, sweep_idx, lat->sc.err, epart, state,
-                                             overlap, st);
+                                             overlap && !lat->slab, st, nullptr, 1, lat->slab ? &lat->sctx : nullptr);
     lat->last_substep = idx;
 }
 
@@ -105,8 +115,9 @@ extern "C" size_t su2_lattice_bytes(int Nx, int Ny, int Nz, int Nt, int precisio
     return (size_t)Nx * Ny * Nz * Nt * 4 * 4 * (precision == 32 ? sizeof(float) : sizeof(double));
 }
 
+// slab_Lt > 0: a time slab with slab_Lt interior slices (Nt = slab_Lt + 4 local slices)
 static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, int nrep, void* dev_links, size_t bytes,
-                       void* stream, bool external, su2_lattice** out)
+                       void* stream, bool external, su2_lattice** out, int slab_Lt = 0)
 {
     if (!out) return SU2_EARG;
     *out = nullptr;
@@ -131,6 +142,8 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, int nrep, 
     g.wup[1] = -(Ny - 1) * g.sy;
     g.wup[2] = -(Nz - 1) * g.sz;
     g.wup[3] = -(Nt - 1) * g.st;
+    g.t_lo = slab_Lt > 0 ? 2 : 0;
+    g.nt_upd = slab_Lt > 0 ? slab_Lt : Nt;
     choose_tiling(g);
     if (g.tile >= 0 && (uint64_t)g.nb[2] * g.nb[3] * nrep > 65535) {  // grid z holds (replica, z-t tile)
         delete lat;
@@ -245,7 +258,9 @@ extern "C" int su2_init(su2_lattice* lat, int start, uint64_t seed)
     ENTER(lat);
     NOT_A_SUBSTEP(lat);
     if (start != SU2_START_COLD && start != SU2_START_HOT) return fail(lat, SU2_EARG, "su2_init: bad start");
-    lat->launches += launch_init(lat->links, lat->g, lat->precision, start, seed, lat->stream);
+    // a slab draws every local slice, halos included, from the global site it is a copy of
+    lat->launches += launch_init(lat->links, lat->g, lat->precision, start, seed, lat->stream,
+                                 lat->slab ? lat->t0 - 2 : 0, lat->slab ? lat->nt_glob : 0);
     CK(lat, cudaGetLastError());
     lat->seed = seed;
     lat->initialised = true;
@@ -311,6 +326,7 @@ extern "C" int su2_batch_sweep_measure(su2_lattice* lat, const double* betas, ui
                                        size_t index)
 {
     ENTER(lat);
+    NOT_ON_A_SLAB(lat, "su2_batch_sweep_measure");
     NOT_A_SUBSTEP(lat);
     if (!betas || !dev_out) return fail(lat, SU2_EARG, "su2_batch_sweep_measure: NULL argument");
     bool changed = false;
@@ -378,6 +394,7 @@ extern "C" int su2_heatbath_substep(su2_lattice* lat, double beta, uint32_t swee
     ENTER(lat);
     if (int rc = check_beta(lat, beta)) return rc;
     if (mu < 0 || mu > 3 || (parity != 0 && parity != 1)) return fail(lat, SU2_EARG, "bad mu / parity");
+    if (lat->slab && !lat->peers_set) return fail(lat, SU2_ESTATE, "slab: su2_slab_set_peers first");
     enqueue_substep(lat, beta, sweep_idx, mu, parity);
     CK(lat, cudaGetLastError());
     return SU2_OK;
@@ -386,6 +403,7 @@ extern "C" int su2_heatbath_substep(su2_lattice* lat, double beta, uint32_t swee
 extern "C" int su2_heatbath_sweep(su2_lattice* lat, double beta, uint32_t sweep_idx)
 {
     ENTER(lat);
+    NOT_ON_A_SLAB(lat, "su2_heatbath_sweep");
     if (int rc = check_beta(lat, beta)) return rc;
     for (int mu = 0; mu < 4; ++mu)      // [R4] direction outer,
         for (int p = 0; p < 2; ++p)     //      parity inner
@@ -398,6 +416,7 @@ extern "C" int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_
                                           size_t index, void* event_after_sweep)
 {
     ENTER(lat);
+    NOT_ON_A_SLAB(lat, "su2_heatbath_sweep_measure");
     if (int rc = check_beta(lat, beta)) return rc;
     if (!dev_out) return fail(lat, SU2_EARG, "su2_heatbath_sweep_measure: NULL dev_out");
     const size_t ctas = heatbath_ctas(lat->g);
@@ -456,6 +475,7 @@ static bool build_run_graph(su2_lattice* lat)
 extern "C" int su2_run(su2_lattice* lat, double beta, uint32_t sweep_idx0, uint32_t n_steps, double* dev_out)
 {
     ENTER(lat);
+    NOT_ON_A_SLAB(lat, "su2_run");
     NOT_A_SUBSTEP(lat);
     if (int rc = check_beta(lat, beta)) return rc;
     if (!dev_out && n_steps) return fail(lat, SU2_EARG, "su2_run: NULL dev_out");
@@ -505,6 +525,7 @@ extern "C" int su2_synchronize(su2_lattice* lat)
 extern "C" int su2_measure_async(su2_lattice* lat, double* dev_out, size_t index)
 {
     ENTER(lat);
+    NOT_ON_A_SLAB(lat, "su2_measure_async");
     NOT_A_SUBSTEP(lat);
     if (!dev_out) return fail(lat, SU2_EARG, "su2_measure_async: NULL dev_out");
     if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
@@ -518,6 +539,7 @@ extern "C" int su2_measure_async(su2_lattice* lat, double* dev_out, size_t index
 extern "C" int su2_measure(su2_lattice* lat, double* plaquette_out, double* polyakov_out)
 {
     ENTER(lat);
+    NOT_ON_A_SLAB(lat, "su2_measure");
     NOT_A_SUBSTEP(lat);
     if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
     if (plaquette_out)
@@ -548,6 +570,7 @@ extern "C" int su2_polyakov_loop(su2_lattice* lat, double* out)
 extern "C" int su2_polyakov_correlator(su2_lattice* lat, int rmax, double* out)
 {
     ENTER(lat);
+    NOT_ON_A_SLAB(lat, "su2_polyakov_correlator");
     NOT_A_SUBSTEP(lat);
     if (!out) return fail(lat, SU2_EARG, "NULL out");
     if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
@@ -605,6 +628,148 @@ extern "C" int su2_set_links(su2_lattice* lat, const void* host_src, size_t byte
     if (ce != cudaSuccess) return fail(lat, SU2_ECUDA, "su2_set_links", ce);
     lat->initialised = true;
     lat->rep_init[lat->selected] = 1;
+    return SU2_OK;
+}
+
+// ---------------------------------------------------------------------------- time slabs
+static bool valid_slab(int Nx, int Ny, int Nz, int Nt, int precision, int t0, int Lt)
+{
+    if (!valid_dims(Nx, Ny, Nz, Nt, precision)) return false;
+    if (Lt < 2 || (Lt & 1) || t0 < 0 || (t0 & 1) || t0 + Lt > Nt) return false;
+    return valid_dims(Nx, Ny, Nz, Lt + 4, precision);
+}
+
+extern "C" size_t su2_slab_bytes(int Nx, int Ny, int Nz, int Lt, int precision)
+{
+    if (Lt < 2 || (Lt & 1)) return 0;
+    return su2_lattice_bytes(Nx, Ny, Nz, Lt + 4, precision);
+}
+
+static int slab_create(int Nx, int Ny, int Nz, int Nt, int precision, int t0, int Lt, void* dev_links, size_t bytes,
+                       void* stream, bool external, su2_lattice** out)
+{
+    if (!out) return SU2_EARG;
+    *out = nullptr;
+    if (!valid_slab(Nx, Ny, Nz, Nt, precision, t0, Lt)) return SU2_EARG;
+    const int rc = create_impl(Nx, Ny, Nz, Lt + 4, precision, 1, dev_links, bytes, stream, external, out, Lt);
+    if (rc != SU2_OK) return rc;
+    su2_lattice* lat = *out;
+    lat->slab = true;
+    lat->nt_glob = Nt;
+    lat->t0 = t0;
+    lat->Lt = Lt;
+    // local slice t holds global slice t0 - 2 + t: site indices differ by (t0 - 2) * NxNyNz (mod 2^32)
+    lat->sctx.s_off = (uint32_t)((int64_t)(t0 - 2) * (int64_t)(2 * lat->g.st));
+    return SU2_OK;
+}
+
+extern "C" int su2_slab_create(int Nx, int Ny, int Nz, int Nt, int precision, int t0, int Lt, su2_lattice** out)
+{
+    return slab_create(Nx, Ny, Nz, Nt, precision, t0, Lt, nullptr, 0, nullptr, false, out);
+}
+
+extern "C" int su2_slab_create_external(int Nx, int Ny, int Nz, int Nt, int precision, int t0, int Lt, void* dev_links,
+                                        size_t bytes, void* cuda_stream, su2_lattice** out)
+{
+    return slab_create(Nx, Ny, Nz, Nt, precision, t0, Lt, dev_links, bytes, cuda_stream, true, out);
+}
+
+extern "C" int su2_slab_set_peers(su2_lattice* lat, void* lo_links, int lo_Lt, void* hi_links, int hi_Lt)
+{
+    ENTER(lat);
+    NOT_A_SUBSTEP(lat);
+    if (!lat->slab) return fail(lat, SU2_ESTATE, "su2_slab_set_peers: not a slab handle");
+    if (!lo_links || !hi_links || lo_Lt < 2 || (lo_Lt & 1) || hi_Lt < 2 || (hi_Lt & 1))
+        return fail(lat, SU2_EARG, "su2_slab_set_peers: bad argument");
+    SlabCtx& c = lat->sctx;
+    c.peer_lo = lo_links;
+    c.peer_hi = hi_links;
+    c.vh_lo = (uint32_t)(lat->g.st * (lo_Lt + 4));
+    c.vh_hi = (uint32_t)(lat->g.st * (hi_Lt + 4));
+    c.d_lo = lo_Lt * lat->g.st;    // own slice 2      -> slice lo_Lt + 2 (upper halo) of the slab below
+    c.d_hi = -lat->Lt * lat->g.st; // own slice Lt + 1 -> slice 1 (lower halo) of the slab above
+    lat->peers_set = true;
+    return SU2_OK;
+}
+
+extern "C" int su2_slab_substep(su2_lattice* lat, double beta, uint32_t sweep_idx, int mu, int parity, int fuse_plaquette)
+{
+    ENTER(lat);
+    if (!lat->slab) return fail(lat, SU2_ESTATE, "su2_slab_substep: not a slab handle");
+    if (int rc = check_beta(lat, beta)) return rc;
+    if (mu < 0 || mu > 3 || (parity != 0 && parity != 1)) return fail(lat, SU2_EARG, "bad mu / parity");
+    if (!lat->peers_set) return fail(lat, SU2_ESTATE, "slab: su2_slab_set_peers first");
+    const size_t ctas = heatbath_ctas(lat->g);
+    enqueue_substep(lat, beta, sweep_idx, mu, parity,
+                    (fuse_plaquette && parity == 1 && mu >= 1) ? lat->sc.epart + (mu - 1) * ctas : nullptr);
+    CK(lat, cudaGetLastError());
+    return SU2_OK;
+}
+
+extern "C" int su2_slab_plaquette(su2_lattice* lat, int fused, double* dev_out)
+{
+    ENTER(lat);
+    NOT_A_SUBSTEP(lat);
+    if (!lat->slab) return fail(lat, SU2_ESTATE, "su2_slab_plaquette: not a slab handle");
+    if (!dev_out) return fail(lat, SU2_EARG, "su2_slab_plaquette: NULL dev_out");
+    if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
+    const double scale = 1.0 / (6.0 * 2.0 * (double)lat->g.st * (double)lat->nt_glob);  // 1 / (6 V_global)
+    if (fused)
+        lat->launches += launch_final_sum(lat->sc.epart, 3 * heatbath_ctas(lat->g), scale, dev_out, lat->stream);
+    else
+        lat->launches += launch_plaquette(lat->links, lat->g, lat->precision, lat->sc, dev_out, lat->stream, scale);
+    CK(lat, cudaGetLastError());
+    return SU2_OK;
+}
+
+extern "C" int su2_slab_polyakov(su2_lattice* lat, const void* dev_prev, void* dev_next, double* dev_out)
+{
+    ENTER(lat);
+    NOT_A_SUBSTEP(lat);
+    if (!lat->slab) return fail(lat, SU2_ESTATE, "su2_slab_polyakov: not a slab handle");
+    if (!lat->initialised) return fail(lat, SU2_ESTATE, "lattice not initialised");
+    if ((dev_prev == nullptr) != (lat->t0 == 0))
+        return fail(lat, SU2_EARG, "su2_slab_polyakov: dev_prev must be NULL exactly on the slab that holds t = 0");
+    if (!dev_next && !dev_out) return fail(lat, SU2_EARG, "su2_slab_polyakov: nothing to write");
+    lat->launches += launch_polyakov_chain(lat->links, lat->g, lat->precision, lat->sc, dev_prev, dev_next, dev_out,
+                                           lat->stream);
+    CK(lat, cudaGetLastError());
+    return SU2_OK;
+}
+
+// CUDA IPC: lets another process (one per GPU) store into this slab's halos
+extern "C" int su2_ipc_export(su2_lattice* lat, void* handle64)
+{
+    ENTER(lat);
+    if (!handle64) return fail(lat, SU2_EARG, "su2_ipc_export: NULL handle buffer");
+    if (!lat->owns_links) return fail(lat, SU2_ESTATE, "su2_ipc_export: the links must be library-allocated (su2_slab_create)");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "cudaIpcMemHandle_t is 64 bytes");
+    cudaIpcMemHandle_t h;
+    CK(lat, cudaIpcGetMemHandle(&h, lat->links_base));
+    memcpy(handle64, &h, sizeof h);
+    return SU2_OK;
+}
+
+extern "C" int su2_ipc_open(const void* handle64, void** dev_ptr)
+{
+    if (!handle64 || !dev_ptr) return SU2_EARG;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle64, sizeof h);
+    if (cudaIpcOpenMemHandle(dev_ptr, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+        cudaGetLastError();
+        *dev_ptr = nullptr;
+        return SU2_ECUDA;
+    }
+    return SU2_OK;
+}
+
+extern "C" int su2_ipc_close(void* dev_ptr)
+{
+    if (!dev_ptr) return SU2_OK;
+    if (cudaIpcCloseMemHandle(dev_ptr) != cudaSuccess) {
+        cudaGetLastError();
+        return SU2_ECUDA;
+    }
     return SU2_OK;
 }
 

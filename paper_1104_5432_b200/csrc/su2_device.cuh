@@ -24,6 +24,9 @@ struct Geom {
     int nb[4];       // tiled launch: number of tiles along hx, y, z, t
     int wup[4];      // half-index delta of +mu at the upper boundary: -(N-1)*stride  (x: -(nxh-1))
     uint32_t zmagic; // ceil(2^32 / nb[2]): blockIdx.z -> (bz, bt) without a division
+    // time slab of a lattice split over GPUs: only the slices t_lo <= t < t_lo + nt_upd
+    // are updated and measured, the others are halo copies. Whole lattice: t_lo = 0, nt_upd = Nt.
+    int t_lo, nt_upd;
 };
 
 // ---------------------------------------------------------------- sites and neighbours
@@ -404,6 +407,13 @@ struct __align__(16) HbParams {
     uint32_t rep_stride;    // links of one configuration: 8 * V/2
     uint32_t nzt;           // tiled launch: CTAs along grid z per replica (nb2 * nb3)
     uint32_t epart_stride;  // fused-plaquette partials per replica (3 * CTAs of one replica)
+    // time slab (ALT kernels only): Philox is keyed by the GLOBAL site, and the links of
+    // the first / last interior slice are also stored into the neighbouring slab's halo (peer memory)
+    uint32_t s_off;                        // global site index - local site index
+    typename LinkPtr<Real>::type* peer_lo;  // array (p,mu) of the slab below (NULL = not a slab)
+    typename LinkPtr<Real>::type* peer_hi;  // array (p,mu) of the slab above
+    int d_lo, d_hi;                        // own link index -> index of its halo copy in peer_lo / peer_hi
+    int t_first, t_last;                   // first / last interior slice (-1 = not a slab)
 };
 
 // [R9] Shoemake: uniform unit quaternion from three uniforms

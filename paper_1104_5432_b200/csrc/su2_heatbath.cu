@@ -44,6 +44,7 @@ struct SiteIdx {
     int h;   // half-index of the site
     int r;   // low bit of x
     int ha;  // h + the replica's offset: index into the link arrays
+    int t;   // time slice (a slab's edge slices are also stored to its neighbours)
 };
 
 template <typename Real>
@@ -125,6 +126,7 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     ix.r = (c.y + c.z + c.t + P) & 1;
     ix.h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
     ix.ha = ix.h + (int)hoff;
+    ix.t = c.t;
     const int h = ix.ha;
     const Nbr d = neighbours(g, c, ix.r);
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
@@ -235,7 +237,8 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
     }
 #endif
     // [R5] counter = (s, sweep, (p<<2)|mu, n); the n = 0 draw does not depend on the links
-    const uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
+    uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
+    if (ALT) s += hp.s_off;  // slab: the global site keys the draws
     const uint32_t tag = ((uint32_t)P << 2) | (uint32_t)MU;
     const Words wd = philox_sel<ALT>(s, sweep, tag, 0u, hp.rk, rc);
 
@@ -304,6 +307,10 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
     const Real inv = M<Real>::rsqrt(u.a0 * u.a0 + u.a1 * u.a1 + u.a2 * u.a2 + u.a3 * u.a3);
     u.a0 *= inv; u.a1 *= inv; u.a2 *= inv; u.a3 *= inv;
     stq(hp.out + (uint32_t)ix.ha, u);
+    if (ALT && hp.peer_lo) {  // slab: the edge slices are the neighbours' halos
+        if (ix.t == hp.t_first) stq(hp.peer_lo + (ix.ha + hp.d_lo), u);
+        if (ix.t == hp.t_last) stq(hp.peer_hi + (ix.ha + hp.d_hi), u);
+    }
     return MEAS ? u.a0 * w.a0 - u.a1 * w.a1 - u.a2 * w.a2 - u.a3 * w.a3 : (Real)0;  // 1/2 Tr(U' w)
 }
 
@@ -365,7 +372,8 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::va
         rep = bzt / hp.nzt;
         bzt -= rep * hp.nzt;
     }
-    const Site c = tile_site<LHX, LY, LZ, LT>(g, bzt);
+    Site c = tile_site<LHX, LY, LZ, LT>(g, bzt);
+    if (ALT) c.t += g.t_lo;  // slab: the grid covers the interior slices only
 #ifdef HB_TMA
     __shared__ __align__(128) typename LinkPtr<Real>::type stage_buf[kTmaSlots << (LHX + LY + LZ + LT)];
     __shared__ __align__(8) uint64_t stage_bar;
@@ -392,9 +400,10 @@ template <typename Real, int MU, int P, bool MEAS, bool ALT>
 __global__ void __launch_bounds__(kBlock)
     heatbath_linear_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
-    const uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
+    uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
     Real e = 0;
-    if (h < g.vh) {
+    if (h < (ALT ? (uint32_t)g.st * (uint32_t)g.nt_upd : g.vh)) {
+        if (ALT) h += (uint32_t)g.st * (uint32_t)g.t_lo;  // slab: interior slices only
         Site c;
         uint32_t q = h / (uint32_t)g.nxh;
         c.hx = (int)(h - q * (uint32_t)g.nxh);
@@ -414,7 +423,8 @@ __global__ void __launch_bounds__(kBlock)
 // [R9] init: one thread per link of the device layout
 template <typename Real>
 __global__ void __launch_bounds__(kBlock)
-    init_kernel(typename LinkPtr<Real>::type* __restrict__ links, const Geom g, int start, uint64_t seed)
+    init_kernel(typename LinkPtr<Real>::type* __restrict__ links, const Geom g, int start, uint64_t seed, int t_shift,
+                int nt_glob)
 {
     const uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
     if (h >= g.vh) return;
@@ -428,7 +438,10 @@ __global__ void __launch_bounds__(kBlock)
         const uint32_t t = q2 / (uint32_t)g.n[2];
         const uint32_t z = q2 - t * (uint32_t)g.n[2];
         const uint32_t r = (y + z + t + (uint32_t)p) & 1u;
-        const uint32_t s = 2u * h + r;
+        // slab: slice t holds the global slice (t + t_shift) mod Nt (t_shift even), whose site keys the draw
+        int tg = ((int)t + t_shift) % nt_glob;
+        if (tg < 0) tg += nt_glob;
+        const uint32_t s = 2u * h + r + 2u * (uint32_t)g.st * (uint32_t)(tg - (int)t);
         const Words w = draw(seed, s, 0u, (1u << 8) | ((uint32_t)p << 2) | (uint32_t)mu, 0u);
         u = haar_from_words<Real>(w);
     }
@@ -442,11 +455,11 @@ void choose_tiling(Geom& g)
     g.zmagic = 0;
     for (int k = 0; k < kNumTiles; ++k) {
         const int* t = kTiles[k];
-        const int ext[4] = {g.nxh, g.n[1], g.n[2], g.n[3]};
+        const int ext[4] = {g.nxh, g.n[1], g.n[2], g.nt_upd};
         bool ok = true;
         for (int d = 0; d < 4; ++d) ok = ok && ext[d] % (1 << t[d]) == 0;
         if (!ok) continue;
-        const uint64_t nb1 = g.n[1] >> t[1], nb2 = g.n[2] >> t[2], nb3 = g.n[3] >> t[3];
+        const uint64_t nb1 = g.n[1] >> t[1], nb2 = g.n[2] >> t[2], nb3 = g.nt_upd >> t[3];
         // grid limits (y, z <= 65535) and exactness of the zmagic split: nb2^2 * nb3 < 2^32
         if (nb1 > 65535 || nb2 * nb3 > 65535) continue;
         g.tile = k;
@@ -462,10 +475,23 @@ void choose_tiling(Geom& g)
 template <typename Real, int MU, int P, bool MEAS, bool ALT>
 static int launch_substep_t(void* links, const Geom& g, double beta, double creutz_below, uint64_t seed,
                             uint32_t sweep, int* err, double* epart, const RunState* state, const RepParams* reps,
-                            int nrep, bool overlap, cudaStream_t st)
+                            int nrep, bool overlap, cudaStream_t st, const SlabCtx* slab)
 {
     typedef typename LinkPtr<Real>::type L;
     HbParams<Real> hp;
+    hp.s_off = 0;
+    hp.peer_lo = hp.peer_hi = nullptr;
+    hp.d_lo = hp.d_hi = 0;
+    hp.t_first = hp.t_last = -1;
+    if (slab) {  // ALT kernels
+        hp.s_off = slab->s_off;
+        hp.peer_lo = (L*)slab->peer_lo + (size_t)(P * 4 + MU) * slab->vh_lo;
+        hp.peer_hi = (L*)slab->peer_hi + (size_t)(P * 4 + MU) * slab->vh_hi;
+        hp.d_lo = slab->d_lo;
+        hp.d_hi = slab->d_hi;
+        hp.t_first = g.t_lo;
+        hp.t_last = g.t_lo + g.nt_upd - 1;
+    }
     hp.inv_beta = (Real)(1.0 / beta);
     hp.sweep = sweep;
     hp.creutz_below = (Real)creutz_below;
@@ -501,17 +527,17 @@ static int launch_substep_t(void* links, const Geom& g, double beta, double creu
 size_t heatbath_ctas(const Geom& g)
 {
     if (g.tile >= 0) return (size_t)g.nb[0] * g.nb[1] * g.nb[2] * g.nb[3];
-    return ((size_t)g.vh + kBlock - 1) / kBlock;
+    return ((size_t)g.st * g.nt_upd + kBlock - 1) / kBlock;
 }
 
 template <typename Real, bool ALT>
 static int launch_substep_p(void* links, const Geom& g, int mu, int parity, double beta, double cb, uint64_t seed,
                             uint32_t sweep, int* err, double* epart, const RunState* state, const RepParams* reps,
-                            int nrep, bool overlap, cudaStream_t st)
+                            int nrep, bool overlap, cudaStream_t st, const SlabCtx* slab)
 {
 #define SU2_HB(MU_, P_, MEAS_, EP_)                                                                               \
     return launch_substep_t<Real, MU_, P_, MEAS_, ALT>(links, g, beta, cb, seed, sweep, err, EP_, state, reps, nrep, \
-                                                       overlap, st)
+                                                       overlap, st, slab)
     if (epart && parity == 1 && mu >= 1) {  // the three measuring kernels
         switch (mu) {
             case 1: SU2_HB(1, 1, true, epart);
@@ -543,25 +569,28 @@ static int launch_substep_p(void* links, const Geom& g, int mu, int parity, doub
 // then holds nrep * 3 * heatbath_ctas(g) partials, replica-major. Batched launches use the ALT kernels.
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
                             double creutz_below, uint64_t seed, uint32_t sweep, int* err, double* epart,
-                            const RunState* state, bool overlap, cudaStream_t st, const RepParams* reps, int nrep)
+                            const RunState* state, bool overlap, cudaStream_t st, const RepParams* reps, int nrep,
+                            const SlabCtx* slab)
 {
-    const bool alt = creutz_below > 0.0 || reps != nullptr;
+    const bool alt = creutz_below > 0.0 || reps != nullptr || slab != nullptr;
     if (!reps) nrep = 1;
 #define SU2_HB(REAL_, ALT_)                                                                                      \
     launch_substep_p<REAL_, ALT_>(links, g, mu, parity, beta, creutz_below, seed, sweep, err, epart, state, reps, \
-                                  nrep, overlap, st)
+                                  nrep, overlap, st, slab)
     if (precision == 32) return alt ? SU2_HB(float, true) : SU2_HB(float, false);
     return alt ? SU2_HB(double, true) : SU2_HB(double, false);
 #undef SU2_HB
 }
 
-int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st)
+int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st, int t_shift,
+                int nt_glob)
 {
     const dim3 grid((g.vh + kBlock - 1) / kBlock, 8);
+    if (nt_glob <= 0) nt_glob = g.n[3];
     if (precision == 32)
-        init_kernel<float><<<grid, kBlock, 0, st>>>((float4*)links, g, start, seed);
+        init_kernel<float><<<grid, kBlock, 0, st>>>((float4*)links, g, start, seed, t_shift, nt_glob);
     else
-        init_kernel<double><<<grid, kBlock, 0, st>>>((double4a*)links, g, start, seed);
+        init_kernel<double><<<grid, kBlock, 0, st>>>((double4a*)links, g, start, seed, t_shift, nt_glob);
     return 1;
 }
 

@@ -55,16 +55,26 @@ struct Scratch {
 };
 constexpr int kMaxR = 128;
 
+// Time slab of a lattice split over GPUs: what a sub-step launch needs beyond Geom.
+struct SlabCtx {
+    uint32_t s_off;          // global site index - local site index (mod 2^32)
+    void* peer_lo;           // [device, possibly peer] link buffer of the slab below
+    void* peer_hi;           // ... of the slab above
+    uint32_t vh_lo, vh_hi;   // links per (p,mu) array of those buffers
+    int d_lo, d_hi;          // own link index -> index of its halo copy there
+};
+
 // fills g.tile (index into kTiles or -1), g.nb and g.zmagic
 void choose_tiling(Geom& g);
 size_t partials_needed(const Geom& g);
 
 // each returns the number of kernels it enqueued (0 on launch failure; check cudaGetLastError)
-int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st);
+int launch_init(void* links, const Geom& g, int precision, int start, uint64_t seed, cudaStream_t st, int t_shift = 0,
+                int nt_glob = 0);
 int launch_heatbath_substep(void* links, const Geom& g, int precision, int mu, int parity, double beta,
                             double creutz_below, uint64_t seed, uint32_t sweep, int* err, double* epart,
                             const RunState* state, bool overlap, cudaStream_t st, const RepParams* reps = nullptr,
-                            int nrep = 1);
+                            int nrep = 1, const SlabCtx* slab = nullptr);
 size_t heatbath_ctas(const Geom& g);
 int launch_final_sum(const double* partials, size_t n, double scale, double* dev_dst, cudaStream_t st);
 int launch_set_run_state(RunState* state, double inv_beta, double* out, uint32_t sweep, uint32_t index,
@@ -75,8 +85,13 @@ int launch_polyakov_partials(const void* links, const Geom& g, int precision, co
 int launch_polyakov_step(const void* links, const Geom& g, int precision, const Scratch& sc, const double* epart,
                          size_t n_epart, double scale_plaq, double* dev_dst, RunState* state, bool overlap,
                          cudaStream_t st, int nrep = 1);
+// `scale` = 0: 1 / (number of plaquettes of g); a slab passes 1 / (plaquettes of the whole lattice)
 int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
-                     cudaStream_t st);
+                     cudaStream_t st, double scale = 0.0);
+// slab: continue the ordered product of time links through the interior slices; prev (nullable) = the
+// product so far per spatial site, next (nullable) = where to store it, dev_dst (nullable) = mean of 1/2 Tr
+int launch_polyakov_chain(const void* links, const Geom& g, int precision, const Scratch& sc, const void* prev,
+                          void* next, double* dev_dst, cudaStream_t st);
 int launch_polyakov(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
                     cudaStream_t st);
 int launch_polyakov_correlator(const Geom& g, const Scratch& sc, int rmax, double* dev_dst, cudaStream_t st);

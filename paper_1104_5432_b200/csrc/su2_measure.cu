@@ -20,10 +20,11 @@ __global__ void __launch_bounds__(kBlock)
 {
     typedef typename LinkPtr<Real>::type L;
     __shared__ double red[kBlock / 32];
-    const uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
+    uint32_t h = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
     const int p = blockIdx.y;
     double acc = 0.0;
-    if (h < g.vh) {
+    if (h < (uint32_t)g.st * (uint32_t)g.nt_upd) {  // = V/2, or the interior slices of a slab
+        h += (uint32_t)g.st * (uint32_t)g.t_lo;
         uint32_t q = h / (uint32_t)g.nxh;
         const int hx = (int)(h - q * (uint32_t)g.nxh);
         uint32_t q2 = q / (uint32_t)g.n[1];
@@ -74,7 +75,8 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), sizeof(Real) == 4 ?
     typedef typename LinkPtr<Real>::type L;
     __shared__ double red[kBlock / 32];
     const int p = blockIdx.x & 1;
-    const Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z, blockIdx.x >> 1);
+    Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z, blockIdx.x >> 1);
+    c.t += g.t_lo;  // slab: interior slices only (0 for a whole lattice)
     const int r = (c.y + c.z + c.t + p) & 1;
     const int h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
     int up[4];
@@ -274,6 +276,48 @@ __global__ void __launch_bounds__(kBlock)
     if (threadIdx.x == 0) partials[blockIdx.x] = tot;
 }
 
+// Time slab: the ordered product continues from slab to slab. `prev` holds the product
+// of the slices below this slab per spatial site (NULL: this slab holds t = 0), `next` receives the
+// product including this slab's interior slices; the association is the plain loop's, left to right.
+template <typename Real>
+__global__ void __launch_bounds__(kBlock)
+    polyakov_chain_kernel(const typename LinkPtr<Real>::type* __restrict__ links, const Geom g,
+                          const typename LinkPtr<Real>::type* __restrict__ prev,
+                          typename LinkPtr<Real>::type* __restrict__ next, double* __restrict__ partials)
+{
+    typedef typename LinkPtr<Real>::type L;
+    __shared__ double red[kBlock / 32];
+    const uint32_t v3 = (uint32_t)g.n[0] * (uint32_t)g.n[1] * (uint32_t)g.n[2];
+    const uint32_t s3 = blockIdx.x * (uint32_t)kBlock + threadIdx.x;
+    double val = 0.0;
+    if (s3 < v3) {
+        const uint32_t x = s3 % (uint32_t)g.n[0];
+        const uint32_t q = s3 / (uint32_t)g.n[0];
+        const uint32_t y = q % (uint32_t)g.n[1], z = q / (uint32_t)g.n[1];
+        const int p0 = (int)((x + y + z) & 1u);
+        const size_t vh = g.vh;
+        const L* a0 = links + (size_t)(p0 * 4 + 3) * vh + (s3 >> 1);        // even t
+        const L* a1 = links + (size_t)((1 - p0) * 4 + 3) * vh + (s3 >> 1);  // odd t
+        int t = g.t_lo;
+        Quat<Real> prod;
+        if (prev) {
+            const L v = prev[s3];
+            prod = {v.x, v.y, v.z, v.w};
+        } else {
+            prod = ldq_cg(((t & 1) ? a1 : a0) + (size_t)t * (size_t)g.st);
+            ++t;
+        }
+        for (; t < g.t_lo + g.nt_upd; ++t) {
+            const Quat<Real> u = ldq_cg(((t & 1) ? a1 : a0) + (size_t)t * (size_t)g.st);
+            prod = qmul<false, false>(prod, u);
+        }
+        val = (double)prod.a0;
+        if (next) stq(next + s3, prod);
+    }
+    const double tot = block_sum(val, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+}
+
 // ------------------------------------------------------------------ correlator (NEXT-1)
 // C(r) = 1/(3 V3) sum_x sum_{i=x,y,z} l(x) l(x + r e_i);  grid.y = r-1
 __global__ void __launch_bounds__(kBlock)
@@ -364,21 +408,21 @@ static void launch_plaquette_t(const void* links, const Geom& g, const Scratch& 
                 <<<grid, 1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3]), 0, st>>>((const L*)links, g,
                                                                                                     sc.partials);
     } else {
-        const dim3 grid(blocks_for(g.vh), 2);
+        const dim3 grid(blocks_for((uint64_t)g.st * g.nt_upd), 2);
         *n_partials = (size_t)grid.x * 2;
         plaquette_kernel<Real><<<grid, kBlock, 0, st>>>((const L*)links, g, sc.partials);
     }
 }
 
 int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
-                     cudaStream_t st)
+                     cudaStream_t st, double scale_in)
 {
     size_t n = 0;
     if (precision == 32)
         launch_plaquette_t<float>(links, g, sc, &n, st);
     else
         launch_plaquette_t<double>(links, g, sc, &n, st);
-    const double scale = 1.0 / (6.0 * 2.0 * (double)g.vh);
+    const double scale = scale_in != 0.0 ? scale_in : 1.0 / (6.0 * 2.0 * (double)g.vh);
     final_sum_kernel<<<1, 1024, 0, st>>>(sc.partials, n, scale, dev_dst);
     return 2;
 }
@@ -462,6 +506,22 @@ int launch_polyakov(const void* links, const Geom& g, int precision, const Scrat
     launch_polyakov_partials(links, g, precision, sc, &n, st);
     const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
     final_sum_kernel<<<1, 1024, 0, st>>>(sc.partials, n, 1.0 / (double)v3, dev_dst);
+    return 2;
+}
+
+int launch_polyakov_chain(const void* links, const Geom& g, int precision, const Scratch& sc, const void* prev,
+                          void* next, double* dev_dst, cudaStream_t st)
+{
+    const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
+    const unsigned grid = blocks_for(v3);
+    if (precision == 32)
+        polyakov_chain_kernel<float><<<grid, kBlock, 0, st>>>((const float4*)links, g, (const float4*)prev, (float4*)next,
+                                                              sc.partials);
+    else
+        polyakov_chain_kernel<double><<<grid, kBlock, 0, st>>>((const double4a*)links, g, (const double4a*)prev,
+                                                               (double4a*)next, sc.partials);
+    if (!dev_dst) return 1;
+    final_sum_kernel<<<1, 1024, 0, st>>>(sc.partials, grid, 1.0 / (double)v3, dev_dst);
     return 2;
 }
 
