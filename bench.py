@@ -276,6 +276,31 @@ def time_aux(pkg, torch, workloads):
         out[f"C2_16^3x4_batch{R}"] = {"us_per_round": dt / n * 1e6, "value": R * w.links * n / dt, "unit": UNIT,
                                       "replicas": R, "precision": 32, "rounds": n}
         bat.close()
+    # time slabs (S8(f) NEXT-4) with every slab on this ONE GPU: the slabs' kernels of a sub-step run one
+    # after the other, so the sweep time is the sum over slabs - what the split costs in kernel time
+    # (ALT kernels, peer stores, no launch overlap), not a multi-GPU number
+    from paper_1104_5432_b200 import slabs
+    w = workloads.BY_NAME["C5_64^4"]
+    for prec in (32, 64):
+        for n_slabs in (2, 4):
+            ring = slabs.SlabRing(w.dims, prec, n_slabs)
+            ring.init(w.start, w.seed)
+            time.sleep(2.0)
+            for k in range(3):
+                ring.sweep(6.0, k)
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            n = 20
+            a.record()
+            for k in range(n):
+                ring.sweep(6.0, 3 + k)
+            b.record()
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b) / n
+            out[f"C5_64^4_fp{prec}_slabs{n_slabs}_on_one_gpu"] = {"ms_per_sweep": ms, "value": w.links / ms * 1e3,
+                                                                 "unit": UNIT, "sweeps": n}
+            ring.close()
+            torch.cuda.empty_cache()
     return out
 
 
