@@ -282,7 +282,12 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
                 const Words w = philox_sel<ALT>(s, sweep, tag, n, hp.rk, rc);
                 delta = M<Real>::kp_delta(w, inv_alpha, tab);
                 const Real Rppp = M<Real>::uniform(w.w3);
+#ifdef HB_PROBE_ONE_TRIAL  // tuning probe (never in the product build; wrong results): every first trial is
+                           // accepted; the time saved bounds what any divergence-limiting scheme could gain
+                if (true) {
+#else
                 if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) {
+#endif
                     delta = M<Real>::kp_delta_refined(w, inv_alpha, delta);
                     break;
                 }
