@@ -301,6 +301,28 @@ def time_aux(pkg, torch, workloads):
                                                                  "unit": UNIT, "sweeps": n}
             ring.close()
             torch.cuda.empty_cache()
+    # the paper's Fig. 1 benchmark over lattice sizes: random SU(2) initialisation, 100
+    # heat-bath iterations at beta = 6.0 with the mean plaquette at each iteration, wall clock of the
+    # whole job (su2_init + one su2_run call, which also takes the Polyakov loop at each iteration)
+    fig1 = []
+    for prec in (32, 64):
+        for L in (8, 16, 24, 32, 48, 64, 96):
+            lat = pkg.Lattice((L, L, L, L), prec)
+            obs = torch.zeros(2 * 100, dtype=torch.float64, device=lat.device)
+            lat.init("hot", 1)
+            lat.run(6.0, 0, 3, obs)  # untimed: graph capture
+            lat.synchronize()
+            time.sleep(1.0)
+            t0 = time.perf_counter()
+            lat.init("hot", 1)
+            lat.run(6.0, 0, 100, obs)
+            lat.synchronize()
+            dt = time.perf_counter() - t0
+            fig1.append({"L": L, "precision": prec, "seconds": dt, "value": 4 * L**4 * 100 / dt, "unit": UNIT,
+                         "plaquette_last": float(obs[198])})
+            lat.close()
+            torch.cuda.empty_cache()
+    out["fig1_init_100_sweeps_plaquette_beta6"] = fig1
     return out
 
 
