@@ -104,10 +104,12 @@ def test_every_substep_matches_oracle_teacher_forced(pkg, dims, prec):
     lat.close()
 
 
-@pytest.mark.parametrize("eps,beta", [(0.05, 6.0), (0.3, 2.3)])
+@pytest.mark.parametrize("eps,beta", [(0.05, 6.0), (0.3, 2.3), (0.01, 100.0), (0.001, 5000.0)])
 @pytest.mark.parametrize("prec", [64, 32])
 def test_sweep_on_smooth_lattice_matches_oracle(pkg, prec, eps, beta):
-    """Thermalised-like inputs (large staple norm, alpha ~ 30 at beta = 6)."""
+    """Thermalised-like inputs (large staple norm, alpha ~ 30 at beta = 6); the last two are the
+    weak-coupling extreme (alpha ~ 600 and ~ 3e4: delta ~ 1/alpha, x0 = 1 - delta within a few ulp of 1
+    in fp32, the direction on a sphere of radius sqrt(2 delta))."""
     dims = (16, 8, 8, 4)
     mode = MODE[prec]
     L = workloads.smooth_links(dims, 9, eps, oracle.dtype(mode))
