@@ -290,7 +290,7 @@ def test_unit_norm_invariant_after_sweeps(pkg, prec):
     lat.close()
 
 
-@pytest.mark.parametrize("beta", [0.3, 1.0])
+@pytest.mark.parametrize("beta", [0.05, 0.3, 1.0])
 def test_fp32_small_alpha_exercises_the_accurate_refinement(pkg, beta):
     """At small alpha = beta*k most accepted trials fall under the kernel's refinement
     threshold (radius^2 < 0.12/alpha^2) and many trials are rejected:
