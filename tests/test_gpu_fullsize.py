@@ -20,6 +20,10 @@ MODE = {64: "f64", 32: "f32"}
     ((64, 64, 64, 64), 32, "cold", 6.0),
     ((64, 64, 64, 64), 64, "cold", 6.0),
     ((48, 48, 48, 6), 64, "hot", 2.5),
+    # grid-limit fall-backs of choose_tiling: 128 x 512 z-t tiles of the first tile shape exceed grid z
+    # (second shape used); Nx = 4 fits neither shape (linear launch over 1M sites)
+    ((32, 8, 256, 512), 32, "hot", 2.3),
+    ((4, 4, 64, 1024), 64, "hot", 2.3),
 ])
 def test_sampled_link_parity_at_bench_sizes(dims, prec, start, beta):
     import paper_1104_5432_b200 as pkg
