@@ -202,7 +202,10 @@ SU2_API int su2_polyakov_correlator(su2_lattice* lat, int rmax, double* out);
 
 /* Configuration I/O in canonical host order (see top). bytes must equal
  * su2_lattice_bytes(...). Both synchronise. su2_set_links marks the lattice initialised.
- * host pointers may be pageable or pinned. */
+ * host pointers may be pageable or pinned. su2_get_links, like su2_synchronize and the measuring
+ * calls, returns SU2_ECUDA if a kernel of the run raised a device-side flag (Kennedy-Pendleton
+ * trial cap; in a -DHB_BOUNDS_CHECK build, a link index outside its array): host_dst is then
+ * filled all the same, the message says which flag. */
 SU2_API int su2_get_links(su2_lattice* lat, void* host_dst, size_t bytes);
 SU2_API int su2_set_links(su2_lattice* lat, const void* host_src, size_t bytes);
 

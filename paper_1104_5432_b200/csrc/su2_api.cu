@@ -512,6 +512,7 @@ static int sync_and_check(su2_lattice* lat)
     CK(lat, cudaMemcpyAsync(&flags, lat->sc.err, sizeof(int), cudaMemcpyDeviceToHost, lat->stream));
     CK(lat, cudaStreamSynchronize(lat->stream));
     if (flags & 1) return fail(lat, SU2_ECUDA, "Kennedy-Pendleton trial cap (10000) hit: alpha = beta*k too small");
+    if (flags & 2) return fail(lat, SU2_ECUDA, "bounds check (HB_BOUNDS_CHECK build): a link index left its array");
     return SU2_OK;
 }
 
@@ -601,9 +602,8 @@ extern "C" int su2_get_links(su2_lattice* lat, void* host_dst, size_t bytes)
     lat->launches += launch_to_canonical(lat->links, stage, g, lat->precision, lat->stream);
     cudaError_t ce = cudaGetLastError();
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(host_dst, stage, need, cudaMemcpyDeviceToHost, lat->stream);
-    if (ce == cudaSuccess) ce = cudaStreamSynchronize(lat->stream);
     if (ce != cudaSuccess) return fail(lat, SU2_ECUDA, "su2_get_links", ce);
-    return SU2_OK;
+    return sync_and_check(lat);  // the links of a run that raised a device-side flag are not handed out silently
 }
 
 extern "C" int su2_set_links(su2_lattice* lat, const void* host_src, size_t bytes)

@@ -109,10 +109,30 @@ __device__ __forceinline__ void tma_row(L* dst, const L* row, int hx0, int sx, i
 }
 #endif
 
+// Checked build (-DHB_BOUNDS_CHECK; compute-sanitizer is not available on the GPU pool): every link index of a
+// heat-bath thread is tested against its array, [hoff, hoff + V/2); a miss sets bit 1 of the error word, which
+// su2_synchronize reports, and the access is redirected to the array's first element.
+#ifdef HB_BOUNDS_CHECK
+__device__ __forceinline__ uint32_t hb_check(uint32_t idx, uint32_t hoff, uint32_t vh, int* err)
+{
+#ifdef HB_BOUNDS_SELFTEST  // proves the check fires: the last element of every array counts as outside
+    vh -= 1;
+#endif
+    if (idx - hoff >= vh) {
+        atomicOr(err, 2);
+        return hoff;
+    }
+    return idx;
+}
+#define HB_CK(idx) hb_check((uint32_t)(idx), hoff, g.vh, err)
+#else
+#define HB_CK(idx) ((uint32_t)(idx))
+#endif
+
 // neighbour addressing (row 2) and the 18 loads (row 3, first half) of one site
 template <typename Real, int MU, int P>
 __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const HbParams<Real>& hp, Staple18<Real>& q,
-                                          uint32_t& sweep, Real& inv_beta, uint32_t hoff
+                                          uint32_t& sweep, Real& inv_beta, uint32_t hoff, int* __restrict__ err
 #ifdef HB_TMA
                                           ,
                                           const TmaStage<Real>* tma = nullptr
@@ -130,7 +150,7 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     const int h = ix.ha;
     const Nbr d = neighbours(g, c, ix.r);
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
-    const uint32_t h_up = (uint32_t)(h + d.up[MU]);
+    const uint32_t h_up = HB_CK(h + d.up[MU]);
 #ifdef HB_TMA
     if (tma) {
         if (threadIdx.x == 0) {
@@ -169,12 +189,12 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
         const int nu = i + (i >= MU ? 1 : 0);
         const L* s_nu = hp.same[nu];
         const L* o_nu = hp.oppo[nu];
-        const uint32_t h_dn = (uint32_t)(h + d.dn[nu]);
-        const uint32_t h_upnu = (uint32_t)(h + d.up[nu]);
+        const uint32_t h_dn = HB_CK(h + d.dn[nu]);
+        const uint32_t h_upnu = HB_CK(h + d.up[nu]);
         TMA_SKIP(TMA_A) q.a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
         TMA_SKIP(TMA_B) q.b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
-        TMA_SKIP(TMA_CC) q.cc[i] = ldq(s_nu + (uint32_t)h);                                  // U_nu(x)
-        TMA_SKIP(TMA_A2) q.a2[i] = ldq(s_nu + (uint32_t)((int)h_up + d.dn[nu]));             // U_nu(x+mu-nu)
+        TMA_SKIP(TMA_CC) q.cc[i] = ldq(s_nu + HB_CK(h));                                      // U_nu(x)
+        TMA_SKIP(TMA_A2) q.a2[i] = ldq(s_nu + HB_CK((int)h_up + d.dn[nu]));               // U_nu(x+mu-nu)
         TMA_SKIP(TMA_B2) q.b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
         TMA_SKIP(TMA_C2) q.c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
         // su2_run's loop state is fetched behind the first six link loads: its round trip then
@@ -336,9 +356,9 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     RepCtx rc = {0u, 0u, hp.rk.k[0], hp.rk.k[1]};
     if (ALT) rc = {rep, rep * hp.rep_stride, hp.rk.k[0], hp.rk.k[1]};
 #ifdef HB_TMA
-    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, rc.hoff, tma);
+    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, rc.hoff, err, tma);
 #else
-    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, rc.hoff);
+    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, rc.hoff, err);
 #endif
     if (ALT && hp.reps) {  // batched launch: this replica's coupling and seed
         const RepParams rp = hp.reps[rep];
