@@ -88,8 +88,19 @@ SU2_API int su2_set_stream(su2_lattice* lat, void* cuda_stream);
 SU2_API int su2_init(su2_lattice* lat, int start, uint64_t seed);
 
 /* Set the seed that keys later sweeps without touching the links (resume from a
- * configuration loaded with su2_set_links). */
+ * configuration loaded with su2_set_links). Takes effect for every later call, su2_run included. */
 SU2_API int su2_set_seed(su2_lattice* lat, uint64_t seed);
+
+/* Launch-structure switches of a handle. They change HOW the kernels are
+ * launched, never what they compute: results are bit-identical with either value (GPU tests).
+ *   SU2_OPT_OVERLAP   1 (default): consecutive sub-steps of a sweep are chained by programmatic
+ *                     dependent launch; 0: every launch fully serialised behind its predecessor.
+ *   SU2_OPT_RUN_GRAPH 1 (default): su2_run replays one captured CUDA graph per step; 0: it enqueues
+ *                     the step's kernels directly.
+ * value must be 0 or 1. Errors: SU2_EARG. */
+#define SU2_OPT_OVERLAP 0
+#define SU2_OPT_RUN_GRAPH 1
+SU2_API int su2_set_option(su2_lattice* lat, int option, int value);
 
 /* Rows 2-6: one full heat-bath sweep = the 8 sub-steps (mu = 0..3 outer, parity 0,1
  * inner) [R4]; each sub-step updates every U_mu(x) of that parity from its Wilson
@@ -171,7 +182,7 @@ SU2_API int su2_run(su2_lattice* lat, double beta, uint32_t sweep_idx0, uint32_t
  * su2_batch_sweep_measure updates all of them with the same 9 launches a single lattice takes, each
  * replica with its own beta and its own seed (its Philox streams are those of a single lattice with that
  * seed).
- *   n_replicas >= 1; n_replicas * 4V < 2^32; (N_z/2 * N_t-tiles) * n_replicas <= 65535.
+ *   1 <= n_replicas <= 65535; n_replicas * 4V < 2^32 (every link of the batch has a 32-bit index).
  * Every single-lattice call (init, sweep, measure, correlator, get/set_links, run ...) works on a batch
  * handle and acts on the SELECTED replica (0 after create). The _external form takes caller-owned
  * memory of n_replicas * su2_lattice_bytes(...) bytes. */

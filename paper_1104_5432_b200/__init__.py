@@ -21,6 +21,7 @@ SU2_OK, SU2_EARG, SU2_EALLOC, SU2_ECUDA, SU2_ESTATE = 0, 1, 2, 3, 4
 SU2_START_COLD, SU2_START_HOT = 0, 1
 SU2_DRAW_KP, SU2_DRAW_AUTO, SU2_DRAW_CREUTZ = 0, 1, 2
 SU2_ALPHA_C = 1.6847
+SU2_OPT_OVERLAP, SU2_OPT_RUN_GRAPH = 0, 1
 
 _lib = None
 
@@ -41,6 +42,7 @@ _SIGNATURES = {
     "su2_init": (C.c_int, [C.c_void_p, C.c_int, C.c_uint64]),
     "su2_set_seed": (C.c_int, [C.c_void_p, C.c_uint64]),
     "su2_set_draw": (C.c_int, [C.c_void_p, C.c_int]),
+    "su2_set_option": (C.c_int, [C.c_void_p, C.c_int, C.c_int]),
     "su2_heatbath_sweep": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32]),
     "su2_heatbath_substep": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32, C.c_int, C.c_int]),
     "su2_heatbath_sweep_measure": (C.c_int, [C.c_void_p, C.c_double, C.c_uint32, C.c_void_p, C.c_size_t,
@@ -171,6 +173,10 @@ def su2_set_seed(h, seed):
 
 def su2_set_draw(h, method):
     _check(lib().su2_set_draw(h, method), h)
+
+
+def su2_set_option(h, option, value):
+    _check(lib().su2_set_option(h, option, int(value)), h)
 
 
 def su2_heatbath_sweep(h, beta, sweep_idx):
@@ -355,6 +361,9 @@ class Lattice:
 
     def set_draw(self, method):
         su2_set_draw(self.h, {"kp": SU2_DRAW_KP, "auto": SU2_DRAW_AUTO, "creutz": SU2_DRAW_CREUTZ}[method])
+
+    def set_option(self, option, value):
+        su2_set_option(self.h, {"overlap": SU2_OPT_OVERLAP, "run_graph": SU2_OPT_RUN_GRAPH}[option], value)
 
     def sweep(self, beta, sweep_idx):
         su2_heatbath_sweep(self.h, beta, sweep_idx)

@@ -24,12 +24,12 @@ struct su2_lattice {
     uint64_t launches;
     int last_substep;  // 2*mu+parity of the heat-bath sub-step that was the LAST work enqueued by this
                        // handle, else -1: decides whether the next sub-step may overlap it
-    bool pdl;          // programmatic dependent launch enabled (SU2HB_NO_PDL=1 disables; A/B timing only)
+    bool pdl;          // programmatic dependent launch enabled (su2_set_option SU2_OPT_OVERLAP)
     // su2_run: one step captured as a CUDA graph, replayed on a private stream
     cudaStream_t run_stream;
     cudaEvent_t run_ev_in, run_ev_out;
     cudaGraphExec_t run_exec;
-    bool run_graphs;   // SU2HB_NO_GRAPH=1 disables (A/B timing only)
+    bool run_graphs;   // su2_run replays a captured CUDA graph (su2_set_option SU2_OPT_RUN_GRAPH)
     double creutz_below;  // [R15] su2_set_draw: 0 (KP), SU2_ALPHA_C (auto) or +inf (Creutz)
     // replica batch: nrep configurations one after the other from links_base; `links`,
     // `seed` and `initialised` are those of the selected replica (single-lattice calls act on it)
@@ -122,8 +122,10 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, int nrep, 
     if (!out) return SU2_EARG;
     *out = nullptr;
     if (!valid_dims(Nx, Ny, Nz, Nt, precision)) return SU2_EARG;
-    // a batch indexes every link of every replica with 32 bits and puts the replica in grid y / z
-    if (nrep < 1 || nrep > 65535 || (uint64_t)nrep * 4ull * Nx * Ny * Nz * Nt >= (1ull << 32)) return SU2_EARG;
+    // a batch indexes every link of every replica with 32 bits and puts the replica in grid y / z; a
+    // single lattice indexes each of its 8 arrays separately (h < V/2), so V < 2^32 is its only limit
+    if (nrep < 1 || nrep > 65535) return SU2_EARG;
+    if (nrep > 1 && (uint64_t)nrep * 4ull * Nx * Ny * Nz * Nt >= (1ull << 32)) return SU2_EARG;
     const size_t rep_bytes = su2_lattice_bytes(Nx, Ny, Nz, Nt, precision);
     const size_t need = rep_bytes * (size_t)nrep;
     if (external && (!dev_links || bytes < need || ((uintptr_t)dev_links & 31))) return SU2_EARG;
@@ -144,21 +146,13 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, int nrep, 
     g.wup[3] = -(Nt - 1) * g.st;
     g.t_lo = slab_Lt > 0 ? 2 : 0;
     g.nt_upd = slab_Lt > 0 ? slab_Lt : Nt;
-    choose_tiling(g);
-    if (g.tile >= 0 && (uint64_t)g.nb[2] * g.nb[3] * nrep > 65535) {  // grid z holds (replica, z-t tile)
-        delete lat;
-        return SU2_EARG;
-    }
+    choose_tiling(g, nrep);  // grid z holds (replica, z-t tile): falls back to the next shape / the linear launch
     lat->nrep = nrep;
     lat->rep_bytes = rep_bytes;
     lat->precision = precision;
     lat->last_substep = -1;
-    {
-        const char* e = getenv("SU2HB_NO_PDL");
-        lat->pdl = !(e && e[0] == '1');
-        e = getenv("SU2HB_NO_GRAPH");
-        lat->run_graphs = !(e && e[0] == '1');
-    }
+    lat->pdl = true;
+    lat->run_graphs = true;
     lat->stream = (cudaStream_t)stream;
     lat->owns_links = !external;
     lat->links = dev_links;
@@ -253,6 +247,31 @@ extern "C" int su2_set_stream(su2_lattice* lat, void* cuda_stream)
     return SU2_OK;
 }
 
+// The captured step of su2_run holds what was current at capture: the link pointers of the selected
+// replica, the expanded Philox keys of the seed, the draw's kernels. Whatever changes one of them drops it.
+static void drop_run_graph(su2_lattice* lat)
+{
+    if (lat->run_exec) {
+        cudaStreamSynchronize(lat->run_stream);
+        cudaGraphExecDestroy(lat->run_exec);
+        lat->run_exec = nullptr;
+    }
+}
+
+extern "C" int su2_set_option(su2_lattice* lat, int option, int value)
+{
+    ENTER(lat);
+    NOT_A_SUBSTEP(lat);
+    if (value != 0 && value != 1) return fail(lat, SU2_EARG, "su2_set_option: value must be 0 or 1");
+    switch (option) {
+        case SU2_OPT_OVERLAP: lat->pdl = value != 0; break;
+        case SU2_OPT_RUN_GRAPH: lat->run_graphs = value != 0; break;
+        default: return fail(lat, SU2_EARG, "su2_set_option: unknown option");
+    }
+    drop_run_graph(lat);  // the captured step was built with the other setting
+    return SU2_OK;
+}
+
 extern "C" int su2_init(su2_lattice* lat, int start, uint64_t seed)
 {
     ENTER(lat);
@@ -262,6 +281,7 @@ extern "C" int su2_init(su2_lattice* lat, int start, uint64_t seed)
     lat->launches += launch_init(lat->links, lat->g, lat->precision, start, seed, lat->stream,
                                  lat->slab ? lat->t0 - 2 : 0, lat->slab ? lat->nt_glob : 0);
     CK(lat, cudaGetLastError());
+    if (seed != lat->seed) drop_run_graph(lat);  // its kernels carry the old seed's round keys
     lat->seed = seed;
     lat->initialised = true;
     lat->rep_seed[lat->selected] = seed;
@@ -272,21 +292,13 @@ extern "C" int su2_init(su2_lattice* lat, int start, uint64_t seed)
 extern "C" int su2_set_seed(su2_lattice* lat, uint64_t seed)
 {
     ENTER(lat);
+    if (seed != lat->seed) drop_run_graph(lat);  // its kernels carry the old seed's round keys
     lat->seed = seed;
     lat->rep_seed[lat->selected] = seed;
     return SU2_OK;
 }
 
 extern "C" int su2_replicas(const su2_lattice* lat) { return lat ? lat->nrep : 0; }
-
-static void drop_run_graph(su2_lattice* lat)
-{
-    if (lat->run_exec) {  // the captured step holds pointers into the replica selected at capture
-        cudaStreamSynchronize(lat->run_stream);
-        cudaGraphExecDestroy(lat->run_exec);
-        lat->run_exec = nullptr;
-    }
-}
 
 extern "C" int su2_select_replica(su2_lattice* lat, int replica)
 {
@@ -307,6 +319,7 @@ extern "C" int su2_batch_init(su2_lattice* lat, int start, const uint64_t* seeds
     NOT_A_SUBSTEP(lat);
     if (start != SU2_START_COLD && start != SU2_START_HOT) return fail(lat, SU2_EARG, "su2_batch_init: bad start");
     if (!seeds) return fail(lat, SU2_EARG, "su2_batch_init: NULL seeds");
+    drop_run_graph(lat);
     for (int r = 0; r < lat->nrep; ++r) {
         lat->launches += launch_init((char*)lat->links_base + (size_t)r * lat->rep_bytes, lat->g, lat->precision, start,
                                      seeds[r], lat->stream);
@@ -373,11 +386,7 @@ extern "C" int su2_set_draw(su2_lattice* lat, int method)
         case SU2_DRAW_CREUTZ: cb = INFINITY; break;
         default: return fail(lat, SU2_EARG, "su2_set_draw: bad method");
     }
-    if (cb != lat->creutz_below && lat->run_exec) {  // the captured step holds the other kernels
-        CK(lat, cudaStreamSynchronize(lat->run_stream));
-        cudaGraphExecDestroy(lat->run_exec);
-        lat->run_exec = nullptr;
-    }
+    if (cb != lat->creutz_below) drop_run_graph(lat);  // the captured step holds the other kernels
     lat->creutz_below = cb;
     return SU2_OK;
 }

@@ -331,7 +331,7 @@ struct M<double> {
     static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
     // su2_math64.cuh: functions specialised to the arguments of this path
     static __device__ __forceinline__ double rsqrt(double x) { return m64::rsqrt_n(x); }  // x normal
-    static __device__ __forceinline__ double sqrt0(double x) { return x * m64::rsqrt_n(fmax(x, 1e-300)); }  // x >= 0
+    static __device__ __forceinline__ double sqrt0(double x) { return m64::sqrt0_n(x); }  // x >= 0
     static __device__ __forceinline__ double cos2pi(double x) { return cospi(2.0 * x); }
     static __device__ __forceinline__ void sincos2pi(double x, double* s, double* c) { sincospi(2.0 * x, s, c); }
     static __device__ __forceinline__ void sincos2pi_word(uint32_t w, double* s, double* c)

@@ -59,55 +59,6 @@ __device__ __forceinline__ void run_state(const HbParams<Real>& hp, uint32_t& sw
     }
 }
 
-#ifdef HB_TMA  // tuning probe (never in the product build): HB_TMA is a mask of the link reads that are
-               // staged through shared memory by TMA bulk copies (cp.async.bulk + mbarrier) instead of
-               // LDGs: bit 0 U_nu(x), 1 U_nu(x-nu), 2 U_mu(x-nu), 3 U_nu(x+mu-nu), 4 U_mu(x+nu),
-               // 5 U_nu(x+mu), each for the three nu. A shifted tile of the CTA is 2^(LY+LZ+LT) contiguous
-               // rows of 2^LHX links (two pieces where a row wraps in x); the row's first thread copies it.
-enum { TMA_CC = 0, TMA_C2 = 1, TMA_B2 = 2, TMA_A2 = 3, TMA_B = 4, TMA_A = 5 };
-__host__ __device__ constexpr int tma_popc(int m) { return m ? (m & 1) + tma_popc(m >> 1) : 0; }
-__host__ __device__ constexpr bool tma_on(int type) { return ((HB_TMA) >> type) & 1; }
-__host__ __device__ constexpr int tma_slot(int type, int i) { return 3 * tma_popc((HB_TMA) & ((1 << type) - 1)) + i; }
-constexpr int kTmaSlots = 3 * tma_popc(HB_TMA);
-template <typename Real>
-struct TmaStage {
-    typename LinkPtr<Real>::type* buf;  // [kTmaSlots][blockDim.x]
-    uint64_t* bar;
-    int row_len;                        // links per contiguous row = 2^LHX
-};
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase)
-{
-    asm volatile(
-        "{\n.reg .pred p;\nWAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(bar)),
-        "r"(phase)
-        : "memory");
-}
-// one row of a shifted tile: links hx0+sx .. hx0+sx+len-1 (mod nxh) of the row at `row` (its hx = 0 element)
-template <typename L>
-__device__ __forceinline__ void tma_row(L* dst, const L* row, int hx0, int sx, int len, int nxh, uint64_t* bar)
-{
-    const int start = hx0 + sx;
-    if (start < 0) {
-        bulk_g2s(dst, row + (nxh - 1), (uint32_t)sizeof(L), bar);
-        bulk_g2s(dst + 1, row, (uint32_t)((len - 1) * sizeof(L)), bar);
-    } else if (start + len > nxh) {
-        bulk_g2s(dst, row + start, (uint32_t)((len - 1) * sizeof(L)), bar);
-        bulk_g2s(dst + (len - 1), row, (uint32_t)sizeof(L), bar);
-    } else {
-        bulk_g2s(dst, row + start, (uint32_t)(len * sizeof(L)), bar);
-    }
-}
-#endif
 
 // Checked build (-DHB_BOUNDS_CHECK; compute-sanitizer is not available on the GPU pool): every link index of a
 // heat-bath thread is tested against its array, [hoff, hoff + V/2); a miss sets bit 1 of the error word, which
@@ -115,9 +66,6 @@ __device__ __forceinline__ void tma_row(L* dst, const L* row, int hx0, int sx, i
 #ifdef HB_BOUNDS_CHECK
 __device__ __forceinline__ uint32_t hb_check(uint32_t idx, uint32_t hoff, uint32_t vh, int* err)
 {
-#ifdef HB_BOUNDS_SELFTEST  // proves the check fires: the last element of every array counts as outside
-    vh -= 1;
-#endif
     if (idx - hoff >= vh) {
         atomicOr(err, 2);
         return hoff;
@@ -132,12 +80,7 @@ __device__ __forceinline__ uint32_t hb_check(uint32_t idx, uint32_t hoff, uint32
 // neighbour addressing (row 2) and the 18 loads (row 3, first half) of one site
 template <typename Real, int MU, int P>
 __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const HbParams<Real>& hp, Staple18<Real>& q,
-                                          uint32_t& sweep, Real& inv_beta, uint32_t hoff, int* __restrict__ err
-#ifdef HB_TMA
-                                          ,
-                                          const TmaStage<Real>* tma = nullptr
-#endif
-)
+                                          uint32_t& sweep, Real& inv_beta, uint32_t hoff, int* __restrict__ err)
 {
     typedef typename LinkPtr<Real>::type L;
     constexpr int DEP_NU = (P == 0) ? (MU + 3) % 4 : -1;
@@ -151,39 +94,6 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     const Nbr d = neighbours(g, c, ix.r);
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
     const uint32_t h_up = HB_CK(h + d.up[MU]);
-#ifdef HB_TMA
-    if (tma) {
-        if (threadIdx.x == 0) {
-            uint64_t st_;
-            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 %0, [%1], %2;"
-                         : "=l"(st_)
-                         : "r"(smem_u32(tma->bar)), "r"((uint32_t)kTmaSlots * blockDim.x * (uint32_t)sizeof(L))
-                         : "memory");
-        }
-        if ((threadIdx.x & (tma->row_len - 1)) == 0) {  // row leader (c.hx = first hx of the tile)
-            const int row0 = h - c.hx;                   // the row's hx = 0 element
-            const int sx_up = ix.r ? 1 : 0, sx_dn = ix.r ? 0 : -1;  // half-index shift of x+1 / x-1
-            const int mu_nonx = (MU == 0) ? 0 : d.up[MU], mu_sx = (MU == 0) ? sx_up : 0;
-#pragma unroll
-            for (int i = 0; i < 3; ++i) {
-                const int nu = i + (i >= MU ? 1 : 0);
-                const int up_nonx = (nu == 0) ? 0 : d.up[nu], up_sx = (nu == 0) ? sx_up : 0;
-                const int dn_nonx = (nu == 0) ? 0 : d.dn[nu], dn_sx = (nu == 0) ? sx_dn : 0;
-                L* base = tma->buf + threadIdx.x;
-                const int n = tma->row_len, nbx = (int)blockDim.x;
-                if (tma_on(TMA_CC)) tma_row(base + tma_slot(TMA_CC, i) * nbx, hp.same[nu] + row0, c.hx, 0, n, g.nxh, tma->bar);
-                if (tma_on(TMA_C2)) tma_row(base + tma_slot(TMA_C2, i) * nbx, hp.oppo[nu] + (row0 + dn_nonx), c.hx, dn_sx, n, g.nxh, tma->bar);
-                if (tma_on(TMA_B2)) tma_row(base + tma_slot(TMA_B2, i) * nbx, o_mu + (row0 + dn_nonx), c.hx, dn_sx, n, g.nxh, tma->bar);
-                if (tma_on(TMA_A2)) tma_row(base + tma_slot(TMA_A2, i) * nbx, hp.same[nu] + (row0 + mu_nonx + dn_nonx), c.hx, mu_sx + dn_sx, n, g.nxh, tma->bar);
-                if (tma_on(TMA_B)) tma_row(base + tma_slot(TMA_B, i) * nbx, o_mu + (row0 + up_nonx), c.hx, up_sx, n, g.nxh, tma->bar);
-                if (tma_on(TMA_A)) tma_row(base + tma_slot(TMA_A, i) * nbx, hp.oppo[nu] + (row0 + mu_nonx), c.hx, mu_sx, n, g.nxh, tma->bar);
-            }
-        }
-    }
-#define TMA_SKIP(type) if (!(tma && tma_on(type)))
-#else
-#define TMA_SKIP(type)
-#endif
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         const int nu = i + (i >= MU ? 1 : 0);
@@ -191,36 +101,16 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
         const L* o_nu = hp.oppo[nu];
         const uint32_t h_dn = HB_CK(h + d.dn[nu]);
         const uint32_t h_upnu = HB_CK(h + d.up[nu]);
-        TMA_SKIP(TMA_A) q.a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
-        TMA_SKIP(TMA_B) q.b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
-        TMA_SKIP(TMA_CC) q.cc[i] = ldq(s_nu + HB_CK(h));                                      // U_nu(x)
-        TMA_SKIP(TMA_A2) q.a2[i] = ldq(s_nu + HB_CK((int)h_up + d.dn[nu]));               // U_nu(x+mu-nu)
-        TMA_SKIP(TMA_B2) q.b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
-        TMA_SKIP(TMA_C2) q.c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
+        q.a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
+        q.b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
+        q.cc[i] = ldq(s_nu + HB_CK(h));                                      // U_nu(x)
+        q.a2[i] = ldq(s_nu + HB_CK((int)h_up + d.dn[nu]));               // U_nu(x+mu-nu)
+        q.b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
+        q.c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
         // su2_run's loop state is fetched behind the first six link loads: its round trip then
         // overlaps theirs instead of preceding them (the n = 0 Philox call needs `sweep`)
         if (i == 0) run_state(hp, sweep, inv_beta);
     }
-#ifdef HB_TMA
-    if (tma) {
-        mbar_wait(tma->bar, 0u);
-        const L* base = tma->buf + threadIdx.x;
-        const int nbx = (int)blockDim.x;
-        auto rd = [&](int type, int i) {
-            const L v = base[tma_slot(type, i) * nbx];
-            return Quat<Real>{v.x, v.y, v.z, v.w};
-        };
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            if (tma_on(TMA_CC)) q.cc[i] = rd(TMA_CC, i);
-            if (tma_on(TMA_C2)) q.c2[i] = rd(TMA_C2, i);
-            if (tma_on(TMA_B2)) q.b2[i] = rd(TMA_B2, i);
-            if (tma_on(TMA_A2)) q.a2[i] = rd(TMA_A2, i);
-            if (tma_on(TMA_B)) q.b[i] = rd(TMA_B, i);
-            if (tma_on(TMA_A)) q.a[i] = rd(TMA_A, i);
-        }
-    }
-#endif
     return ix;
 }
 
@@ -242,20 +132,6 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
 {
     const Quat<Real>*a = q.a, *b = q.b, *cc = q.cc, *a2 = q.a2, *b2 = q.b2, *c2 = q.c2;
     const int h = ix.h, r = ix.r;
-#ifdef HB_PROBE_MEMONLY  // tuning probe (never in the product build): the 18 loads, a sum, the store
-    {
-        Quat<Real> sacc = {0, 0, 0, 0};
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            sacc.a0 += a[i].a0 + b[i].a0 + cc[i].a0 + a2[i].a0 + b2[i].a0 + c2[i].a0;
-            sacc.a1 += a[i].a1 + b[i].a1 + cc[i].a1 + a2[i].a1 + b2[i].a1 + c2[i].a1;
-            sacc.a2 += a[i].a2 + b[i].a2 + cc[i].a2 + a2[i].a2 + b2[i].a2 + c2[i].a2;
-            sacc.a3 += a[i].a3 + b[i].a3 + cc[i].a3 + a2[i].a3 + b2[i].a3 + c2[i].a3;
-        }
-        stq(hp.out + (uint32_t)ix.ha, sacc);
-        return (Real)0;
-    }
-#endif
     // [R5] counter = (s, sweep, (p<<2)|mu, n); the n = 0 draw does not depend on the links
     uint32_t s = 2u * (uint32_t)h + (uint32_t)r;
     if (ALT) s += hp.s_off;  // slab: the global site keys the draws
@@ -302,12 +178,7 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
                 const Words w = philox_sel<ALT>(s, sweep, tag, n, hp.rk, rc);
                 delta = M<Real>::kp_delta(w, inv_alpha, tab);
                 const Real Rppp = M<Real>::uniform(w.w3);
-#ifdef HB_PROBE_ONE_TRIAL  // tuning probe (never in the product build; wrong results): every first trial is
-                           // accepted; the time saved bounds what any divergence-limiting scheme could gain
-                if (true) {
-#else
                 if (Rppp * Rppp <= (Real)1 - (Real)0.5 * delta) {
-#endif
                     delta = M<Real>::kp_delta_refined(w, inv_alpha, delta);
                     break;
                 }
@@ -341,12 +212,7 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
 
 template <typename Real, int MU, int P, bool MEAS, bool ALT>
 __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp, uint32_t rep,
-                                              int* __restrict__ err
-#ifdef HB_TMA
-                                              ,
-                                              const TmaStage<Real>* tma = nullptr
-#endif
-)
+                                              int* __restrict__ err)
 {
     grid_dep_wait();    // the preceding kernel of the stream has finished and flushed
     grid_dep_launch();  // ... so the next one may be scheduled behind this CTA
@@ -355,11 +221,7 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     Staple18<Real> q;
     RepCtx rc = {0u, 0u, hp.rk.k[0], hp.rk.k[1]};
     if (ALT) rc = {rep, rep * hp.rep_stride, hp.rk.k[0], hp.rk.k[1]};
-#ifdef HB_TMA
-    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, rc.hoff, err, tma);
-#else
     const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, rc.hoff, err);
-#endif
     if (ALT && hp.reps) {  // batched launch: this replica's coupling and seed
         const RepParams rp = hp.reps[rep];
         inv_beta = (Real)rp.inv_beta;
@@ -399,19 +261,7 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::va
     }
     Site c = tile_site<LHX, LY, LZ, LT>(g, bzt);
     if (ALT) c.t += g.t_lo;  // slab: the grid covers the interior slices only
-#ifdef HB_TMA
-    __shared__ __align__(128) typename LinkPtr<Real>::type stage_buf[kTmaSlots << (LHX + LY + LZ + LT)];
-    __shared__ __align__(8) uint64_t stage_bar;
-    if (threadIdx.x == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&stage_bar)) : "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __syncthreads();  // ahead of griddepcontrol.wait: overlaps the predecessor's tail
-    const TmaStage<Real> tma = {stage_buf, &stage_bar, 1 << LHX};
-    const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err, &tma);
-#else
     const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err);
-#endif
     if (MEAS) {  // one fp64 partial per CTA, fixed order
         __shared__ double red[kBlock / 32];
         const double tot = block_sum_end(e, red);
@@ -473,7 +323,7 @@ __global__ void __launch_bounds__(kBlock)
     stq(links + (size_t)arr * g.vh + h, u);
 }
 
-void choose_tiling(Geom& g)
+void choose_tiling(Geom& g, int nrep)
 {
     g.tile = -1;
     g.nb[0] = g.nb[1] = g.nb[2] = g.nb[3] = 0;
@@ -486,7 +336,8 @@ void choose_tiling(Geom& g)
         if (!ok) continue;
         const uint64_t nb1 = g.n[1] >> t[1], nb2 = g.n[2] >> t[2], nb3 = g.nt_upd >> t[3];
         // grid limits (y, z <= 65535) and exactness of the zmagic split: nb2^2 * nb3 < 2^32
-        if (nb1 > 65535 || nb2 * nb3 > 65535) continue;
+        // (a batch carries the replica in grid z as well)
+        if (nb1 > 65535 || nb2 * nb3 * (uint64_t)nrep > 65535) continue;
         g.tile = k;
         g.nb[0] = g.nxh >> t[0];
         g.nb[1] = (int)nb1;

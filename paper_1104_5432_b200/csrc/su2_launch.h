@@ -64,8 +64,8 @@ struct SlabCtx {
     int d_lo, d_hi;          // own link index -> index of its halo copy there
 };
 
-// fills g.tile (index into kTiles or -1), g.nb and g.zmagic
-void choose_tiling(Geom& g);
+// fills g.tile (index into kTiles or -1), g.nb and g.zmagic; nrep = replicas of a batch (grid z = replica x z-t tiles)
+void choose_tiling(Geom& g, int nrep = 1);
 size_t partials_needed(const Geom& g);
 
 // each returns the number of kernels it enqueued (0 on launch failure; check cudaGetLastError)

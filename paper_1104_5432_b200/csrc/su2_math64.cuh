@@ -13,6 +13,7 @@
 //   cos2_2pi_uniform(w) cos^2(2 pi (w + 1/2) 2^-32)   fold to (0, pi/4), one sine polynomial
 //   sincos_2pi_uniform  sin, cos of the same angle     octant fold, sine + cosine polynomial
 //   rsqrt_n(x)          1/sqrt(x), x normal            MUFU.RSQ64H + one cubic iteration
+//   sqrt0_n(x)          sqrt(x), x >= 0                 x * rsqrt_n(max(x, 1e-300))
 //
 // All are __host__ __device__ so that a host harness can check them against libm.
 #pragma once
@@ -188,6 +189,17 @@ __host__ __device__ __forceinline__ double rsqrt_n(double x)
     const double e = SU2_M64_FMA(-(x * y), y, 1.0);
     const double t = SU2_M64_FMA(e, 0.375, 0.5);
     return SU2_M64_FMA(y * e, t, y);
+}
+
+// sqrt(x) for x >= 0 as x * rsqrt(x); the clamp keeps rsqrt_n's argument normal, so that
+// sqrt0_n(0) = 0 exactly and a denormal x gives a value below 1e-150 instead of a NaN.
+__host__ __device__ __forceinline__ double sqrt0_n(double x)
+{
+#if defined(__CUDA_ARCH__)
+    return x * rsqrt_n(fmax(x, 1e-300));
+#else
+    return x * rsqrt_n(x > 1e-300 ? x : 1e-300);
+#endif
 }
 
 }  // namespace m64

@@ -17,7 +17,7 @@ int main(int argc, char** argv)
 {
     const long n = argc > 1 ? atol(argv[1]) : 4000000L;
     const long double PI = 3.141592653589793238462643383279502884L;
-    double log_rel = 0, cos2_abs = 0, sincos_abs = 0, rsqrt_rel = 0;
+    double log_rel = 0, cos2_abs = 0, sincos_abs = 0, rsqrt_rel = 0, sqrt0_rel = 0;
     uint64_t st = 88172645463325252ull;  // xorshift64: test inputs only
     for (long i = 0; i < n; ++i) {
         st ^= st << 13; st ^= st >> 7; st ^= st << 17;
@@ -36,8 +36,14 @@ int main(int argc, char** argv)
         const double x = ldexp(1.0 + u, (int)(w % 80) - 60);
         const long double rr = 1.0L / sqrtl((long double)x);
         rsqrt_rel = fmax(rsqrt_rel, fabs((double)((rsqrt_n(x) - rr) / rr)));
+        // sqrt0_n over the arguments the kernel gives it: delta (2 - delta) and 1 - cos^2(theta), both in [0, 1],
+        // down to the smallest positive values (u^2 ~ 1e-20) - the function M<double>::sqrt0 calls
+        const double y0 = (i & 1) ? u * u : u * (2.0 - u) * 0.5;
+        const long double sr = sqrtl((long double)y0);
+        sqrt0_rel = fmax(sqrt0_rel, fabs((double)((sqrt0_n(y0) - sr) / sr)));
     }
-    printf("log_rel %.3e cos2_abs %.3e sincos_abs %.3e rsqrt_rel %.3e sqrt0_zero %.3e sqrt_tiny %.17g\n", log_rel,
-           cos2_abs, sincos_abs, rsqrt_rel, 0.0 * rsqrt_n(1e-300), 1e-300 * rsqrt_n(1e-300));
+    printf("log_rel %.3e cos2_abs %.3e sincos_abs %.3e rsqrt_rel %.3e sqrt0_rel %.3e sqrt0_zero %.3e sqrt0_denormal %.3e "
+           "sqrt_tiny %.17g\n",
+           log_rel, cos2_abs, sincos_abs, rsqrt_rel, sqrt0_rel, sqrt0_n(0.0), sqrt0_n(4.9e-324), sqrt0_n(1e-300));
     return 0;
 }

@@ -332,14 +332,14 @@ def test_substeps_in_any_order_match_oracle(pkg):
 
 
 @pytest.mark.parametrize("prec", [64, 32])
-def test_overlapped_launches_equal_serialised_launches_bitwise(pkg, prec, monkeypatch):
+def test_overlapped_launches_equal_serialised_launches_bitwise(pkg, prec):
     """32^4 (many CTA waves): sweeps whose sub-steps are chained by programmatic dependent
     launch give bit-identical links to the same sweeps with the overlap disabled."""
     dims = (32, 32, 32, 32)
     res = []
-    for no_pdl in ("0", "1"):
-        monkeypatch.setenv("SU2HB_NO_PDL", no_pdl)
+    for overlap in (1, 0):
         lat = pkg.Lattice(dims, prec)
+        lat.set_option("overlap", overlap)
         lat.init("hot", 2)
         for i in range(3):
             lat.sweep(6.0, i)
@@ -398,14 +398,14 @@ def test_sweep_measure_fused_plaquette_matches_oracle_and_standalone_kernel(pkg,
 @pytest.mark.parametrize("graphs", ["1", "0"])
 @pytest.mark.parametrize("prec", [64, 32])
 @pytest.mark.parametrize("dims", [(16, 8, 8, 4), (32, 4, 4, 2), (8, 8, 8, 8), (6, 4, 10, 2)])
-def test_run_equals_step_by_step_calls_bitwise(pkg, dims, prec, graphs, monkeypatch):
+def test_run_equals_step_by_step_calls_bitwise(pkg, dims, prec, graphs):
     """su2_run (captured CUDA graph replayed n times, loop state in device memory) against n
     su2_heatbath_sweep_measure calls: identical links and observables; also with the graph
     disabled (direct launches reading the same device state)."""
     import torch
-    monkeypatch.setenv("SU2HB_NO_GRAPH", "0" if graphs == "1" else "1")
     n = 7
     a, b = pkg.Lattice(dims, prec), pkg.Lattice(dims, prec)
+    b.set_option("run_graph", int(graphs))
     oa = torch.zeros(2 * n, dtype=torch.float64, device="cuda")
     ob = torch.zeros(2 * n, dtype=torch.float64, device="cuda")
     for lat in (a, b):
@@ -506,6 +506,56 @@ def test_run_follows_set_draw_and_bad_method_is_rejected(pkg):
     with pytest.raises(pkg.SU2Error):
         pkg.su2_set_draw(a.h, 7)
     a.close(); b.close()
+
+
+@pytest.mark.parametrize("how", ["set_seed", "init"])
+def test_run_after_reseed_uses_the_new_seed(pkg, how):
+    """The captured step of su2_run carries the seed's expanded Philox keys as kernel parameters:
+    a reseed (su2_set_seed, or su2_init with another seed) must drop it. run(seed A); reseed B;
+    run must equal the step-by-step calls with seed B, bit for bit."""
+    import torch
+    dims, prec, beta, n = (16, 8, 8, 4), 64, 2.3, 3
+    a, b = pkg.Lattice(dims, prec), pkg.Lattice(dims, prec)
+    oa = torch.zeros(4 * n, dtype=torch.float64, device="cuda")
+    ob = torch.zeros(4 * n, dtype=torch.float64, device="cuda")
+    a.init("hot", 1)
+    b.init("hot", 1)
+    a.run(beta, 0, n, oa)                       # captures the step with seed 1
+    for i in range(n):
+        b.sweep_measure(beta, i, ob, i)
+    if how == "set_seed":
+        a.set_seed(2)
+        b.set_seed(2)
+    else:
+        a.init("hot", 2)
+        b.init("hot", 2)
+    a.run(beta, n, n, oa[2 * n:])
+    for i in range(n):
+        b.sweep_measure(beta, n + i, ob, n + i)
+    torch.cuda.synchronize()
+    assert (a.get_links() == b.get_links()).all()
+    assert torch.equal(oa, ob)
+    # ... and the oracle agrees on which stream that is
+    if how == "init":
+        L = oracle.init(dims, "hot", 2, "f64")
+        for i in range(n):
+            oracle.heatbath_sweep(dims, L, beta, 2, n + i, "f64")
+        assert_links_match(a.get_links(), L, 64)
+    a.close(); b.close()
+
+
+def test_set_option_rejects_bad_arguments(pkg):
+    lat = pkg.Lattice((4, 4, 4, 4), 32)
+    for opt, val in ((7, 1), (pkg.SU2_OPT_OVERLAP, 2), (pkg.SU2_OPT_RUN_GRAPH, -1)):
+        with pytest.raises(pkg.SU2Error) as e:
+            pkg.su2_set_option(lat.h, opt, val)
+        assert e.value.code == pkg.SU2_EARG
+    lat.set_option("overlap", 0)
+    lat.set_option("run_graph", 0)
+    lat.init("cold", 1)
+    lat.sweep(2.3, 0)
+    assert 0.0 < lat.mean_plaquette() <= 1.0
+    lat.close()
 
 
 # ---------------------------------------------------------------- replica batches (S8(f) NEXT-2)

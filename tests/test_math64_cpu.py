@@ -30,7 +30,9 @@ def test_math64_against_libm(tmp_path):
     assert r["cos2_abs"] < 5e-16
     assert r["sincos_abs"] < 3e-16
     assert r["rsqrt_rel"] < 3e-16
-    assert r["sqrt0_zero"] == 0.0      # sqrt0(0) = 0 * rsqrt(1e-300)
+    assert r["sqrt0_rel"] < 3e-16      # m64::sqrt0_n itself (the function M<double>::sqrt0 calls)
+    assert r["sqrt0_zero"] == 0.0      # exactly 0 at 0, no NaN
+    assert 0.0 <= r["sqrt0_denormal"] < 1e-150
     assert abs(r["sqrt_tiny"] - 1e-150) < 1e-165
 
 
