@@ -33,7 +33,7 @@ def lib():
             f.restype = areal
             for name in ("orc_init", "orc_staple", "orc_staple_norms", "orc_kp_x0", "orc_creutz_x0", "orc_set_draw", "orc_heatbath_link",
                          "orc_heatbath_substep", "orc_heatbath_sweep", "orc_mean_plaquette",
-                         "orc_plaquette_at", "orc_polyakov_loop", "orc_gauge_transform"):
+                         "orc_plaquette_at", "orc_polyakov_loop", "orc_polyakov_correlator", "orc_gauge_transform"):
                 getattr(_lib, f"{name}_{m}").restype = C.c_int
             getattr(_lib, f"orc_qmul_{m}").restype = None
     return _lib
@@ -132,36 +132,40 @@ def set_draw(method, mode="f64"):
     _check(getattr(lib(), f"orc_set_draw_{mode}")(DRAW[method]), "set_draw")
 
 
-def heatbath_link(dims, links, beta, seed, sweep, s, mu, mode="f64"):
+def heatbath_link(dims, links, beta, seed, sweep, s, mu, mode="f64", return_k=False):
+    """New link of (site s, direction mu), lattice untouched. Returns (u, trials, margin[, k])."""
     D, d = _dims(dims)
     u = np.zeros(4, dtype=_DT[mode])
     tr = C.c_int(0)
     mg = C.c_double(0)
+    kn = C.c_double(0)
     rc = getattr(lib(), f"orc_heatbath_link_{mode}")(D, _p(d), _p(links), C.c_double(beta), C.c_uint64(seed),
                                                     C.c_uint32(sweep), C.c_int64(s), mu, _p(u), C.byref(tr),
-                                                    C.byref(mg))
+                                                    C.byref(mg), C.byref(kn))
     _check(rc, "heatbath_link")
-    return u, tr.value, mg.value
+    return (u, tr.value, mg.value, kn.value) if return_k else (u, tr.value, mg.value)
 
 
-def heatbath_substep(dims, links, beta, seed, sweep, mu, parity, mode="f64", order=None, trials=None, margin=None):
-    """In place on `links`."""
+def heatbath_substep(dims, links, beta, seed, sweep, mu, parity, mode="f64", order=None, trials=None, margin=None,
+                     knorm=None):
+    """In place on `links`. trials: int32 [V][D]; margin, knorm (staple norm k of each updated link):
+    float64 [V][D]; all optional, only the entries of the updated links are written."""
     D, d = _dims(dims)
     assert links.dtype == _DT[mode] and links.flags.c_contiguous
     if order is not None:
         order = np.ascontiguousarray(order, dtype=np.int64)
     rc = getattr(lib(), f"orc_heatbath_substep_{mode}")(D, _p(d), _p(links), C.c_double(beta), C.c_uint64(seed),
                                                        C.c_uint32(sweep), mu, parity, _p(order), _p(trials),
-                                                       _p(margin))
+                                                       _p(margin), _p(knorm))
     _check(rc, "heatbath_substep")
 
 
-def heatbath_sweep(dims, links, beta, seed, sweep, mode="f64", trials=None, margin=None):
-    """In place on `links`. trials: int32 [V][D]; margin: float64 [V][D] (both optional)."""
+def heatbath_sweep(dims, links, beta, seed, sweep, mode="f64", trials=None, margin=None, knorm=None):
+    """In place on `links`. trials: int32 [V][D]; margin, knorm: float64 [V][D] (all optional)."""
     D, d = _dims(dims)
     assert links.dtype == _DT[mode] and links.flags.c_contiguous
     rc = getattr(lib(), f"orc_heatbath_sweep_{mode}")(D, _p(d), _p(links), C.c_double(beta), C.c_uint64(seed),
-                                                     C.c_uint32(sweep), _p(trials), _p(margin))
+                                                     C.c_uint32(sweep), _p(trials), _p(margin), _p(knorm))
     _check(rc, "heatbath_sweep")
 
 
@@ -187,6 +191,15 @@ def polyakov_loop(dims, links, mode="f64", return_field=False):
     rc = getattr(lib(), f"orc_polyakov_loop_{mode}")(D, _p(d), _p(links), C.byref(out), _p(field))
     _check(rc, "polyakov_loop")
     return (out.value, field) if return_field else out.value
+
+
+def polyakov_correlator(dims, links, rmax, mode="f64"):
+    """C(r) = <l(x) l(x + r e_i)> over all spatial x and the D-1 spatial axes, r = 1..rmax (eq. 3)."""
+    D, d = _dims(dims)
+    out = np.zeros(rmax, dtype=np.float64)
+    rc = getattr(lib(), f"orc_polyakov_correlator_{mode}")(D, _p(d), _p(links), int(rmax), _p(out))
+    _check(rc, "polyakov_correlator")
+    return out
 
 
 def gauge_transform(dims, links, seed, mode="f64"):

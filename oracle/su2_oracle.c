@@ -33,7 +33,10 @@
  * heat bath on 2^4 vs brute-force quadrature; cold plaquette = 1; gauge
  * invariance; Polyakov centre flip; D=2 equilibrium plaquette = I2(b)/I1(b);
  * D=4 Schwinger–Dyson identity; visiting-order independence; Creutz draw [R15]
- * vs I2/I1, (pi/2) I1/sinh and the quadrature CDF.
+ * vs I2/I1, (pi/2) I1/sinh and the quadrature CDF; the staple norm k returned
+ * beside the margin vs the norm of the (pinned) staple; Polyakov-loop correlator:
+ * cold C(r) = 1, a field with one non-trivial line, gauge invariance,
+ * C(r) = C(N - r), factorisation on x-independent configurations.
  * Unpinned: D=4 <L> values across the N_t=4 transition (the paper prints none).
  */
 #include <math.h>
@@ -454,8 +457,13 @@ int FN(orc_creutz_x0)(double alpha, uint64_t seed, uint32_t s, uint32_t sweep, d
 #define DEGENERATE_K2 1e-30
 #endif
 
+/* *knorm (nullable) = the staple norm k of this link as the update saw it: the draw divides the
+ * staple by it (Vbar = v/k), so 1/k is the factor by which a perturbation of the neighbouring
+ * links reaches the new link - the parity harness classifies ill-conditioned links with it
+ * (DESIGN.md 3 [R13b]). */
 static int heatbath_link(const geom_t *g, const REAL *links, double beta, uint64_t seed,
-                         uint32_t sweep, int64_t s, int mu, AREAL unew[4], int *trials, AREAL *margin)
+                         uint32_t sweep, int64_t s, int mu, AREAL unew[4], int *trials, AREAL *margin,
+                         double *knorm)
 {
     int x[ORC_MAXD];
     site_coords(g, s, x);
@@ -471,9 +479,11 @@ static int heatbath_link(const geom_t *g, const REAL *links, double beta, uint64
         haar_from_words(wd, unew);
         if (trials) *trials = 0;
         if (margin) *margin = (AREAL)1;
+        if (knorm) *knorm = 0.0;
         return ORC_OK;
     }
     AREAL k = A_SQRT(k2);
+    if (knorm) *knorm = (double)k;
     AREAL alpha = (AREAL)beta * k;
 
     AREAL delta;
@@ -514,12 +524,13 @@ static int heatbath_link(const geom_t *g, const REAL *links, double beta, uint64
 
 /* one link, result returned, lattice untouched (single-link pins) */
 int FN(orc_heatbath_link)(int D, const int *dims, const REAL *links, double beta, uint64_t seed,
-                          uint32_t sweep, int64_t s, int mu, REAL *u_out, int *trials, double *margin)
+                          uint32_t sweep, int64_t s, int mu, REAL *u_out, int *trials, double *margin,
+                          double *knorm)
 {
     geom_t g;
     if (geom_init(&g, D, dims) || s < 0 || s >= g.V || mu < 0 || mu >= D || !(beta > 0)) return ORC_EARG;
     AREAL u[4], m;
-    int rc = heatbath_link(&g, links, beta, seed, sweep, s, mu, u, trials, &m);
+    int rc = heatbath_link(&g, links, beta, seed, sweep, s, mu, u, trials, &m, knorm);
     if (rc) return rc;
     for (int c = 0; c < 4; ++c) u_out[c] = (REAL)u[c];
     if (margin) *margin = (double)m;
@@ -529,10 +540,10 @@ int FN(orc_heatbath_link)(int D, const int *dims, const REAL *links, double beta
 /* One sub-step (mu, parity) [R4]: every U_mu(x) with parity(x) = parity, in
  * place. `order` (nullable) is a permutation of 0..V-1 giving the visiting
  * order of the sites (order-independence pin); NULL = ascending s.
- * trials/margin (nullable) are indexed [s*D+mu]. */
+ * trials/margin/knorm (nullable) are indexed [s*D+mu]. */
 int FN(orc_heatbath_substep)(int D, const int *dims, REAL *links, double beta, uint64_t seed,
                              uint32_t sweep, int mu, int parity, const int64_t *order,
-                             int32_t *trials, double *margin)
+                             int32_t *trials, double *margin, double *knorm)
 {
     geom_t g;
     if (geom_init(&g, D, dims) || mu < 0 || mu >= D || (parity != 0 && parity != 1) || !(beta > 0) ||
@@ -545,23 +556,26 @@ int FN(orc_heatbath_substep)(int D, const int *dims, REAL *links, double beta, u
         if (site_parity(&g, x) != parity) continue;
         AREAL u[4], m;
         int tr;
-        int rc = heatbath_link(&g, links, beta, seed, sweep, s, mu, u, &tr, &m);
+        double kn;
+        int rc = heatbath_link(&g, links, beta, seed, sweep, s, mu, u, &tr, &m, &kn);
         if (rc) return rc;
         REAL *dst = links + (s * D + mu) * 4;
         for (int c = 0; c < 4; ++c) dst[c] = (REAL)u[c];
         if (trials) trials[s * D + mu] = tr;
         if (margin) margin[s * D + mu] = (double)m;
+        if (knorm) knorm[s * D + mu] = kn;
     }
     return ORC_OK;
 }
 
 /* One sweep [R4]: for mu = 0..D-1: for parity = 0, 1: sub-step(mu, parity). */
 int FN(orc_heatbath_sweep)(int D, const int *dims, REAL *links, double beta, uint64_t seed,
-                           uint32_t sweep, int32_t *trials, double *margin)
+                           uint32_t sweep, int32_t *trials, double *margin, double *knorm)
 {
     for (int mu = 0; mu < D; ++mu)
         for (int parity = 0; parity < 2; ++parity) {
-            int rc = FN(orc_heatbath_substep)(D, dims, links, beta, seed, sweep, mu, parity, NULL, trials, margin);
+            int rc = FN(orc_heatbath_substep)(D, dims, links, beta, seed, sweep, mu, parity, NULL, trials, margin,
+                                              knorm);
             if (rc) return rc;
         }
     return ORC_OK;
@@ -663,6 +677,58 @@ int FN(orc_polyakov_loop)(int D, const int *dims, const REAL *links, double *out
         neumaier_add(&sum, &comp, (double)prod[0]);
     }
     *out = (sum + comp) / (double)Vs;
+    return ORC_OK;
+}
+
+/* ====================================================================== */
+/* Polyakov-loop correlator (eq. 3): the colour-averaged free */
+/* energy is defined through 1/4 <Tr L(y) Tr L^dag(x)>. In SU(2) Tr L is real, */
+/* so 1/4 Tr L(y) Tr L^dag(x) = l(y) l(x) with l = 1/2 Tr L as in [R11].      */
+/* On-axis separations only (SURVEY.md 8(f) item 1 - the paper does not say   */
+/* which separations it used): for r = 1..rmax                                */
+/*   C(r) = 1/((D-1) Vs) sum_xs sum_{i spatial} l(xs) l(xs + r e_i), periodic. */
+/* Written as the direct double loop over sites and axes, on the field l that */
+/* orc_polyakov_loop defines (recomputed here the same way, product over t in */
+/* order); sums in double with Neumaier compensation. out[r-1] = C(r).        */
+/* ====================================================================== */
+int FN(orc_polyakov_correlator)(int D, const int *dims, const REAL *links, int rmax, double *out)
+{
+    geom_t g;
+    if (geom_init(&g, D, dims) || !links || !out || rmax < 1) return ORC_EARG;
+    int td = D - 1;
+    for (int i = 0; i < td; ++i)
+        if (rmax > g.n[i] / 2) return ORC_EARG;
+    int64_t Vs = g.V / g.n[td];
+    double *l = (double *)malloc(sizeof(double) * (size_t)Vs);
+    if (!l) return ORC_EARG;
+    for (int64_t xs = 0; xs < Vs; ++xs) { /* l(xs) = 1/2 Tr prod_t U_t(xs, t) [R11] */
+        int x[ORC_MAXD];
+        site_coords(&g, xs, x);
+        AREAL prod[4] = {1, 0, 0, 0};
+        for (int t = 0; t < g.n[td]; ++t) {
+            x[td] = t;
+            AREAL u[4], nxt[4];
+            load_link(&g, links, x, td, u);
+            qmul(prod, u, nxt);
+            for (int c = 0; c < 4; ++c) prod[c] = nxt[c];
+        }
+        l[xs] = (double)prod[0];
+    }
+    for (int r = 1; r <= rmax; ++r) {
+        double sum = 0.0, comp = 0.0;
+        for (int64_t xs = 0; xs < Vs; ++xs) {
+            int x[ORC_MAXD];
+            site_coords(&g, xs, x);
+            for (int i = 0; i < td; ++i) {
+                int y[ORC_MAXD];
+                for (int e = 0; e < D; ++e) y[e] = x[e];
+                y[i] = (x[i] + r) % g.n[i];
+                neumaier_add(&sum, &comp, l[xs] * l[site_index(&g, y)]);
+            }
+        }
+        out[r - 1] = (sum + comp) / ((double)td * (double)Vs);
+    }
+    free(l);
     return ORC_OK;
 }
 

@@ -15,6 +15,7 @@ import numpy as np
 import pytest
 
 import oracle
+import parity_protocol as pp
 from paper_1104_5432_b200 import workloads
 
 pytestmark = pytest.mark.gpu
@@ -22,7 +23,6 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 TOL = {64: 1e-12, 32: 1e-5}
 PTOL = {64: 1e-12, 32: 1e-6}
-FLIP_MARGIN = {64: 1e-11, 32: 1e-5}
 MODE = {64: "f64", 32: "f32"}
 
 
@@ -85,12 +85,9 @@ def test_slab_substeps_match_oracle_teacher_forced(pkg, slabs, dims, n, prec):
             ring.substep(beta, sweep, mu, p)
             g = ring.get_links()
             o = L.copy()
-            mg = np.ones((V, 4))
-            oracle.heatbath_substep(dims, o, beta, seed, sweep, mu, p, mode, margin=mg)
-            d = np.abs(g.astype(np.float64) - o.astype(np.float64)).max(-1)
-            bad = d > TOL[prec]
-            assert (mg[bad] < FLIP_MARGIN[prec]).all() and bad.sum() <= (0 if prec == 64 else 1), \
-                f"mu={mu} p={p}: {int(bad.sum())} links differ, max {d.max():.3e}"
+            mg, kn = np.ones((V, 4)), np.ones((V, 4))
+            oracle.heatbath_substep(dims, o, beta, seed, sweep, mu, p, mode, margin=mg, knorm=kn)
+            pp.compare_links(g, o, dims, prec, [(mu, p)], mg, kn, what=f"mu={mu} p={p}")  # DESIGN.md 3 [R13], [R13b]
             untouched = np.ones((V, 4), bool)
             untouched[par == p, mu] = False
             assert (g[untouched] == L[untouched]).all()

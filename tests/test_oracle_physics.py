@@ -427,3 +427,126 @@ def test_d2_equilibrium_plaquette_with_creutz_draw(draw_mode):
     vals = np.array(vals)
     b = vals[: len(vals) // 20 * 20].reshape(20, -1).mean(1)
     assert abs(vals.mean() - 0.240194) < 4.5 * b.std(ddof=1) / np.sqrt(20)
+
+
+# ---------------------------------------------------------------- staple norm k returned beside the margin ([R13b])
+@pytest.mark.parametrize("mode", ["f64", "f32"])
+def test_returned_staple_norm_is_the_norm_of_the_pinned_staple(mode):
+    """heatbath_substep(knorm=...) hands out the k of every link it updates. It must be the
+    quaternion norm of the staple sum of the PRE-update lattice - orc_staple, which the
+    plaquette-sum identity above pins - and only the updated entries may be written.
+    orc_staple_norms (all links at once) must agree with the same values."""
+    dims = [4, 6, 4, 2]
+    L = workloads.random_links(dims, 17, oracle.dtype(mode))
+    V = oracle.volume(dims)
+    for mu, p in ((0, 1), (3, 0)):
+        before = L.copy()
+        all_k = oracle.staple_norms(dims, before, mode)
+        kn = np.full((V, 4), -7.0)
+        oracle.heatbath_substep(dims, L, 2.3, 5, 0, mu, p, mode, knorm=kn)
+        s = np.arange(V)
+        par = (s % 4 + s // 4 % 6 + s // 24 % 4 + s // 96) % 2
+        written = kn != -7.0
+        assert written[par == p, mu].all() and written.sum() == (par == p).sum()
+        tol = 1e-14 if mode == "f64" else 1e-6
+        for site in np.flatnonzero(par == p)[::5]:
+            v = oracle.staple(dims, before, int(site), mu, mode).astype(np.float64)
+            assert abs(kn[site, mu] - np.linalg.norm(v)) < tol
+            assert abs(all_k[site, mu] - np.linalg.norm(v)) < tol
+        u, tr, mg, k1 = oracle.heatbath_link(dims, before, 2.3, 5, 0, int(site), mu, mode, return_k=True)
+        assert k1 == kn[site, mu]
+    # the hand-built k = 0 link [R8] reports k = 0
+    Z = workloads.degenerate_staple_links((4, 4, 4, 4), 37, 1, oracle.dtype(mode))
+    assert oracle.heatbath_link((4, 4, 4, 4), Z, 2.3, 5, 0, 37, 1, mode, return_k=True)[3] == 0.0
+
+
+# ---------------------------------------------------------------- Polyakov-loop correlator (PAPER.md:80-85, eq. 3)
+def _with_time_link(dims, sites_and_quats):
+    """cold lattice whose time link at (xs, t = 1) is the given unit quaternion: l(xs) = its a0"""
+    V = oracle.volume(dims)
+    L = np.zeros((V, 4, 4))
+    L[..., 0] = 1.0
+    Vs = V // dims[3]
+    for xs, q in sites_and_quats:
+        L[Vs * 1 + xs, 3] = np.asarray(q) / np.linalg.norm(q)
+    return L
+
+
+def test_correlator_cold_and_constant_field():
+    dims = [6, 4, 8, 4]
+    L = oracle.init(dims, "cold", 0)
+    assert (oracle.polyakov_correlator(dims, L, 2) == 1.0).all()
+    # every time link on slice 2 equal to one quaternion q: l(x) = q0 everywhere, C(r) = q0^2
+    q = np.array([0.3, -0.5, 0.1, 0.8])
+    q /= np.linalg.norm(q)
+    Lr = L.reshape(4, -1, 4, 4)
+    Lr[2, :, 3] = q
+    assert np.abs(oracle.polyakov_correlator(dims, L, 2) - q[0] ** 2).max() < 1e-15
+
+
+def test_correlator_counts_the_pairs_of_two_nontrivial_lines():
+    """Cold lattice with two Polyakov lines of value a and b a distance d = 2 apart along y. Of the
+    3 Vs ordered pairs (x, x + r e_i), 6 contain the first line and 6 the second; for r = d one pair
+    contains both. So C(r) = (3Vs - 12 + 6a + 6b)/(3Vs) for r != d and (3Vs - 11 + 5a + 5b + ab)/(3Vs)
+    for r = d: pins the normalisation, the axis loop, the direction of the shift and the r index."""
+    dims = [8, 8, 6, 4]
+    nx, ny, nz, _ = dims
+    Vs = nx * ny * nz
+    x0 = 3 + nx * (1 + ny * 2)
+    x1 = 3 + nx * (3 + ny * 2)
+    qa, qb = [0.6, 0.8, 0.0, 0.0], [-0.28, 0.0, 0.96, 0.0]
+    L = _with_time_link(dims, [(x0, qa), (x1, qb)])
+    a, b = 0.6, -0.28
+    C = oracle.polyakov_correlator(dims, L, 3)
+    plain = (3 * Vs - 12 + 6 * a + 6 * b) / (3 * Vs)
+    both = (3 * Vs - 11 + 5 * a + 5 * b + a * b) / (3 * Vs)
+    assert np.abs(C - [plain, both, plain]).max() < 1e-15
+    # the same two lines 2 apart along z, on a lattice with Nz = 6: r = 2 only (r = 3 = Nz/2 does not see it)
+    x1z = 3 + nx * (1 + ny * 4)
+    C = oracle.polyakov_correlator(dims, _with_time_link(dims, [(x0, qa), (x1z, qb)]), 3)
+    assert np.abs(C - [plain, both, plain]).max() < 1e-15
+    # wrapped the other way: lines 6 apart along x on Nx = 8 are 2 apart
+    x1x = (3 + 6) % nx + nx * (1 + ny * 2)
+    C = oracle.polyakov_correlator(dims, _with_time_link(dims, [(x0, qa), (x1x, qb)]), 3)
+    assert np.abs(C - [plain, both, plain]).max() < 1e-15
+
+
+def test_correlator_is_gauge_invariant_and_equals_the_fft_autocorrelation():
+    """Eq. 3 'is gauge invariant'; and by Wiener-Khinchin the periodic autocorrelation of
+    the field l along one axis is the inverse FFT of |FFT l|^2 - a library route that shares nothing
+    with the double loop (the field itself is pinned by the centre-flip and 2x2-matrix tests)."""
+    dims = [8, 6, 10, 4]
+    L = oracle.init(dims, "hot", 12)
+    for i in range(2):
+        oracle.heatbath_sweep(dims, L, 2.6, 12, i)
+    C = oracle.polyakov_correlator(dims, L, 3)
+    G = L.copy()
+    oracle.gauge_transform(dims, G, 9)
+    assert np.abs(oracle.polyakov_correlator(dims, G, 3) - C).max() < 1e-14
+    _, field = oracle.polyakov_loop(dims, L, return_field=True)
+    f = field.reshape(dims[2], dims[1], dims[0])  # [z][y][x]
+    want = np.zeros(3)
+    for ax in range(3):
+        F = np.fft.fft(f, axis=ax)
+        ac = np.fft.ifft(F * np.conj(F), axis=ax).real  # sum_x l(x) l(x + r) along ax, at index r
+        want += np.array([np.take(ac, r, axis=ax).sum() for r in (1, 2, 3)])
+    want /= 3 * f.size
+    assert np.abs(C - want).max() < 1e-14
+    # C(r) = C(N - r): on the mirrored lattice (x -> -x, which maps U_t(x) to U_t(-x)) the values are the same
+    Lm = L.reshape(dims[3], dims[2], dims[1], dims[0], 4, 4)[:, :, :, ::-1]
+    M = np.zeros_like(L).reshape(Lm.shape)
+    M[..., 3, :] = Lm[..., 3, :]     # only the time links enter; the others stay zero (never read)
+    M[..., :3, 0] = 1.0
+    assert np.abs(oracle.polyakov_correlator(dims, np.ascontiguousarray(M).reshape(L.shape), 3) - C).max() < 1e-14
+
+
+def test_correlator_rejects_bad_rmax_and_fp32_mode_tracks_fp64():
+    dims = [4, 6, 4, 2]
+    L = workloads.random_links(dims, 3, np.float64)
+    with pytest.raises(RuntimeError):
+        oracle.polyakov_correlator(dims, L, 3)      # > min extent / 2
+    with pytest.raises(RuntimeError):
+        oracle.polyakov_correlator(dims, L, 0)
+    a = oracle.polyakov_correlator(dims, L, 2)
+    b = oracle.polyakov_correlator(dims, L.astype(np.float32), 2, "f32")
+    assert np.abs(a - b).max() < 2e-7

@@ -1,0 +1,143 @@
+"""The comparison protocol itself (tests/parity_protocol.py) on the CPU: its dependency geometry is
+pinned against the oracle (which links change when one link is perturbed), and its verdicts on
+hand-made deviations are the ones DESIGN.md §3 [R13]/[R13b] states."""
+import numpy as np
+import pytest
+
+import oracle
+import parity_protocol as pp
+from paper_1104_5432_b200 import workloads
+
+
+@pytest.mark.parametrize("dims", [(4, 6, 4, 2), (2, 2, 2, 2), (4, 4, 4, 4)])
+def test_staple_dependency_geometry_matches_the_oracle(dims):
+    """Perturb one link; the links of sub-step (mu, p) that the oracle then computes differently are
+    exactly those whose staple [R3] contains it - what staple_inputs_any() predicts."""
+    nx, ny, nz, nt = dims
+    V = oracle.volume(dims)
+    L = workloads.random_links(dims, 4, np.float64)
+    rng = np.random.default_rng(1)
+    par = pp.parity_grid(dims)
+    for trial in range(6):
+        s0, nu0 = int(rng.integers(V)), int(rng.integers(4))
+        Lp = L.copy()
+        Lp[s0, nu0] = workloads.random_links((2, 2, 2, 2), 100 + trial)[0, 0]
+        flag = np.zeros((V, 4), bool)
+        flag[s0, nu0] = True
+        flag = flag.reshape(nt, nz, ny, nx, 4)
+        for mu in range(4):
+            for p in range(2):
+                a, b = L.copy(), Lp.copy()
+                oracle.heatbath_substep(dims, a, 2.3, 9, 0, mu, p)
+                oracle.heatbath_substep(dims, b, 2.3, 9, 0, mu, p)
+                changed = (np.abs(a - b).max(-1) > 0).reshape(nt, nz, ny, nx, 4)
+                changed[flag] = False   # the perturbed link itself (overwritten if it is in the sub-step)
+                want = pp.staple_inputs_any(flag, mu) & (par == p)
+                assert np.array_equal(changed[..., mu], want), (trial, mu, p)
+                others = np.delete(changed, mu, axis=-1)
+                assert not others.any()
+
+
+def _sweep_records(dims, mode, seed=3, beta=2.3):
+    L = workloads.random_links(dims, 8, oracle.dtype(mode))
+    V = oracle.volume(dims)
+    mg, kn = np.ones((V, 4)), np.ones((V, 4))
+    oracle.heatbath_sweep(dims, L, beta, seed, 0, mode, margin=mg, knorm=kn)
+    return L, mg, kn
+
+
+def test_protocol_verdicts_on_hand_made_deviations():
+    dims, prec = (8, 4, 4, 4), 32
+    ora, mg, kn = _sweep_records(dims, "f32")
+    V = oracle.volume(dims)
+    # identical and within-tolerance results are clean
+    assert pp.compare_links(ora, ora, dims, prec, pp.SWEEP, mg, kn).clean
+    near = ora + np.float32(3e-6)
+    assert pp.compare_links(near, ora, dims, prec, pp.SWEEP, mg, kn).clean
+    # an O(1) deviation with a healthy margin and a healthy k has no excuse
+    s, mu = 77, 3   # direction 3 is updated last: nothing is downstream of it
+    assert mg[s, mu] > 1e-3 and kn[s, mu] > 0.5
+    gpu = ora.copy()
+    gpu[s, mu] = -gpu[s, mu]
+    with pytest.raises(AssertionError, match="no excuse"):
+        pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, mg, kn)
+    # the same deviation with a marginal accept decision is one flip ...
+    m2 = mg.copy()
+    m2[s, mu] = 3e-7
+    r = pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, m2, kn)
+    assert (r.flips, r.small_k, r.downstream) == (1, 0, 0)
+    # ... two such links exceed the budget of a 2048-link sweep
+    gpu2 = gpu.copy()
+    gpu2[s + 2, mu] = -gpu2[s + 2, mu]
+    m2[s + 2, mu] = 1e-7
+    with pytest.raises(AssertionError, match="budget"):
+        pp.compare_links(gpu2, ora, dims, prec, pp.SWEEP, m2, kn)
+    # a flip in an early sub-step excuses what is downstream of it, and only that
+    s1, mu1 = 40, 0
+    gpu = ora.copy()
+    gpu[s1, mu1] = -gpu[s1, mu1]
+    m3 = mg.copy()
+    m3[s1, mu1] = 1e-8
+    nx, ny, nz, nt = dims
+    flag = np.zeros((nt, nz, ny, nx, 4), bool)
+    flag.reshape(V, 4)[s1, mu1] = True
+    par = pp.parity_grid(dims)
+    p1 = int(par.reshape(-1)[s1])
+    hit = pp.staple_inputs_any(flag, 1) & (par == 1 - p1)       # links of sub-step (1, 1 - p1) that read it
+    idx = np.flatnonzero(hit.reshape(-1))
+    assert len(idx) > 0
+    gpu[idx[0], 1] = -gpu[idx[0], 1]
+    r = pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, m3, kn)
+    assert (r.flips, r.downstream) == (1, 1)
+    far = int(np.flatnonzero(~hit.reshape(-1) & (par.reshape(-1) == 1 - p1))[-1])
+    gpu[far, 1] = -gpu[far, 1]
+    with pytest.raises(AssertionError, match="no excuse"):
+        pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, m3, kn)
+
+
+def test_small_k_excuse_scales_with_one_over_k_and_is_fp32_only():
+    dims = (8, 4, 4, 4)
+    ora, mg, kn = _sweep_records(dims, "f32")
+    s, mu = 90, 3
+    k2 = kn.copy()
+    k2[s, mu] = 0.02                      # E_V / k = 5e-5
+    gpu = ora.copy()
+    gpu[s, mu, 1] += np.float32(4e-5)
+    r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k2)
+    assert (r.flips, r.small_k) == (0, 1)
+    gpu[s, mu, 1] += np.float32(4e-5)     # 8e-5 > E_V / k: more than 1/k explains
+    with pytest.raises(AssertionError, match="no excuse"):
+        pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k2)
+    # fp64 has no small-k excuse and a zero flip budget
+    o64, m64, k64 = _sweep_records(dims, "f64")
+    g64 = o64.copy()
+    g64[s, mu, 1] += 1e-11
+    k64[s, mu] = 1e-4
+    with pytest.raises(AssertionError, match="no excuse"):
+        pp.compare_links(g64, o64, dims, 64, pp.SWEEP, m64, k64)
+    m64[s, mu] = 1e-13
+    with pytest.raises(AssertionError, match="budget"):
+        pp.compare_links(g64, o64, dims, 64, pp.SWEEP, m64, k64)
+
+
+def test_budgets():
+    assert pp.flip_budget(65536, 64) == 0 and pp.small_k_budget(65536, 64) == 0
+    assert pp.flip_budget(16, 32) == 1 and pp.flip_budget(65536, 32) == 1
+    assert pp.flip_budget(4 * 32**4, 32) == int(np.ceil(5 * pp.FLIP_RATE[32] * 4 * 32**4))
+    assert pp.small_k_budget(65536, 32) == 2 and pp.small_k_budget(65536, 32, haar=False) == 1
+
+
+def test_fp32_oracle_modes_agree_under_the_protocol():
+    """The oracle's two fp32 modes (float arithmetic vs double arithmetic on float storage, [R12]) play
+    'GPU' and 'oracle': a real pair of roundings of the same update must pass the protocol."""
+    dims = (8, 8, 4, 4)
+    L = workloads.random_links(dims, 2, np.float32)
+    V = oracle.volume(dims)
+    a, b = L.copy(), L.copy()
+    mg, kn = np.ones((V, 4)), np.ones((V, 4))
+    oracle.heatbath_sweep(dims, a, 2.3, 4, 1, "f32x")
+    oracle.heatbath_sweep(dims, b, 2.3, 4, 1, "f32", margin=mg, knorm=kn)
+    r = pp.compare_links(a, b, dims, 32, pp.SWEEP, mg, kn)
+    assert r.flips <= 1
+    pp.check_observables(oracle.mean_plaquette(dims, a, "f32x"), oracle.polyakov_loop(dims, a, "f32x"), a, dims, 32,
+                         rep=r, ora_links=b)
