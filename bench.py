@@ -159,12 +159,46 @@ def dist_env():
 
 
 # ------------------------------------------------------------------------------- ours
-def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, dist=None):
-    """Device-resident timing of `steps` steps. Returns a dict of measurements."""
+def _sweep_leg(lat, torch, beta, obs, idx0, n, every=1, dist=None, sampler=None):
+    """`n` consecutive su2_heatbath_sweep_measure calls, timed on the device as a whole, with a CUDA-event
+    pair around the 8 sub-step kernels of every `every`-th step (the second event of a pair is recorded by
+    the library between the 8th sub-step and the reduction kernel): the heat-bath kernel's average launch
+    duration for the roofline comes from the SAME region as the step time."""
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    pairs = {k: (ev(), ev()) for k in range(0, n, every)}
+    for a, b in pairs.values():  # materialise the CUDA events (torch creates them on first record)
+        a.record()
+        b.record()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    n0 = lat.launch_count
+    t0 = sampler.mark() if sampler else 0.0
+    start, stop = ev(), ev()
+    start.record()
+    for k in range(n):
+        if k in pairs:
+            pairs[k][0].record()
+            lat.sweep_measure(beta, idx0 + k, obs, idx0 + k, pairs[k][1])
+        else:
+            lat.sweep_measure(beta, idx0 + k, obs, idx0 + k)
+    stop.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t1 = sampler.mark() if sampler else 0.0
+    lat.synchronize()  # surfaces device-side error flags
+    return {"ms_total": start.elapsed_time(stop), "steps": n, "launches": int(lat.launch_count - n0),
+            "sweep_ms": float(np.mean([a.elapsed_time(b) for a, b in pairs.values()])), "t_wall": (t0, t1)}
+
+
+def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, dist=None, sustained_s=1.0):
+    """Device-resident timing. Burst leg: EXACTLY `steps` steps after a cool-down and `warmup` untimed steps
+    (the line's `value`). Sustained leg: a continuous run of the same steps, the first third untimed (the GPU
+    reaches its power-capped state), then >= `sustained_s` seconds timed. Returns a dict of measurements."""
     time.sleep(COOL_DOWN_S)  # every workload starts from the same power state, whatever ran before it
     lat = pkg.Lattice(w.dims, prec)
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    obs = torch.zeros(2 * (steps + warmup), dtype=torch.float64, device=lat.device)
 
     e0, e1 = ev(), ev()
     torch.cuda.synchronize()
@@ -174,61 +208,57 @@ def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, 
     torch.cuda.synchronize()
     init_ms = e0.elapsed_time(e1)
 
-    # warm-up, then the timed region: EXACTLY `steps` steps, one su2_heatbath_sweep_measure call
-    # each, with a CUDA-event pair around the 8 sub-step kernels of every step (the second
-    # event of a pair is recorded by the library between the 8th sub-step and the reductions):
-    # the heat-bath kernel's average launch duration for the roofline comes from the SAME region
+    obs = torch.zeros(2 * (steps + warmup), dtype=torch.float64, device=lat.device)
     for i in range(warmup):
         lat.sweep_measure(beta, i, obs, i)
     lat.synchronize()
-    sweep_ev = [(ev(), ev()) for _ in range(steps)]
-    for a, b in sweep_ev:  # materialise the CUDA events (torch creates them on first record)
-        a.record()
-        b.record()
-    if dist is not None:
-        dist.barrier()
-    torch.cuda.synchronize()
-    n0 = lat.launch_count
-    t_wall0 = sampler.mark() if sampler else 0.0
-    start, stop = ev(), ev()
-    start.record()
-    for k in range(steps):
-        sweep_ev[k][0].record()
-        lat.sweep_measure(beta, warmup + k, obs, warmup + k, sweep_ev[k][1])
-    stop.record()
-    torch.cuda.synchronize()
-    if dist is not None:
-        dist.barrier()
-    t_wall1 = sampler.mark() if sampler else 0.0
-    lat.synchronize()  # surfaces device-side error flags
-    launches = lat.launch_count - n0
-    ms = start.elapsed_time(stop)
-    sweep_ms = float(np.mean([a.elapsed_time(b) for a, b in sweep_ev]))
+    burst = _sweep_leg(lat, torch, beta, obs, warmup, steps, 1, dist, sampler)
     o = obs.cpu().numpy().reshape(-1, 2).copy()
 
-    # extra (not the headline): the same `steps` steps as ONE su2_run call — the step captured as
+    res = {"ms_total": burst["ms_total"], "ms_per_step": burst["ms_total"] / steps, "sweep_ms": burst["sweep_ms"],
+           "init_ms": init_ms, "launches": burst["launches"], "plaquette_last": float(o[warmup + steps - 1, 0]),
+           "polyakov_last": float(o[warmup + steps - 1, 1]), "t_wall": burst["t_wall"], "links": w.links}
+
+    if sustained_s > 0:
+        n_sus = max(steps, int(np.ceil(sustained_s * 1e3 / res["ms_per_step"] * 1.1)))
+        n_pre = max(warmup, n_sus // 3)
+        obs2 = torch.zeros(2 * (n_pre + n_sus), dtype=torch.float64, device=lat.device)
+        base = warmup + steps
+        for i in range(n_pre):  # untimed: continuous load until the power cap has settled
+            lat.sweep_measure(beta, base + i, obs2, i)
+        sus = _sweep_leg(lat, torch, beta, _Shifted(obs2, base), base + n_pre, n_sus, max(1, n_sus // 200), dist,
+                         sampler)
+        res["sustained"] = {"ms_total": sus["ms_total"], "steps": n_sus, "ms_per_step": sus["ms_total"] / n_sus,
+                            "sweep_ms": sus["sweep_ms"], "t_wall": sus["t_wall"], "untimed_steps_before": n_pre}
+        del obs2
+
+    # extra (not the headline): the same `steps` steps as ONE su2_run call - the step captured as
     # a CUDA graph and replayed, no host work per step (matters on small lattices)
-    time.sleep(COOL_DOWN_S)  # same power state as the timed region above started from
-    lat.run(beta, warmup + steps, min(warmup, steps), obs)  # captures the graph
+    time.sleep(COOL_DOWN_S)  # same power state as the burst leg started from
+    lat.run(beta, 1 << 20, min(warmup, steps), obs)  # captures the graph
     torch.cuda.synchronize()
     s2, e2 = ev(), ev()
     s2.record()
-    lat.run(beta, warmup + steps, steps, obs)
+    lat.run(beta, (1 << 20) + warmup, steps, obs)
     e2.record()
     torch.cuda.synchronize()
     lat.synchronize()
-    ms_run = s2.elapsed_time(e2) / steps
-    res = {
-        "ms_total": ms, "ms_per_step": ms / steps, "sweep_ms": sweep_ms, "init_ms": init_ms,
-        "ms_per_step_run": ms_run,
-        "launches": int(launches), "plaquette_last": float(o[warmup + steps - 1, 0]),
-        "polyakov_last": float(o[warmup + steps - 1, 1]), "t_wall": (t_wall0, t_wall1),
-        "links": w.links,
-    }
+    res["ms_per_step_run"] = s2.elapsed_time(e2) / steps
     lat.close()
     del lat, obs
     torch.cuda.empty_cache()
     return res
+
+
+class _Shifted:
+    """A device tensor addressed with the sweep index minus `base` (su2_heatbath_sweep_measure takes the
+    output slot and the sweep index separately; the sustained leg continues the chain's sweep indices)."""
+
+    def __init__(self, t, base):
+        self.t, self.base = t, base
+
+    def data_ptr(self):
+        return self.t.data_ptr() - 16 * self.base
 
 
 def time_aux(pkg, torch, workloads):

@@ -285,6 +285,21 @@ SU2_API int su2_ipc_export(su2_lattice* lat, void* handle64);
 SU2_API int su2_ipc_open(const void* handle64, void** dev_ptr);
 SU2_API int su2_ipc_close(void* dev_ptr);
 
+/* Measurement support: memory bandwidth of the current device with the
+ * access shape of the path - 128-bit loads, unit stride across a warp, every SM busy, no arithmetic - over a
+ * zero-filled scratch buffer of `bytes` (>= 1 MiB, multiple of 32) that the call allocates and frees.
+ *   mode SU2_PROBE_READ: every pass reads the buffer once. With bytes <= L2 (64 MiB = the 32^4 fp32 lattice
+ *        in the 126 MB L2) the passes after the two untimed ones are served by L2: the L2 roofline
+ *        denominator of the cache-resident point of the metric. With bytes >> L2: HBM read bandwidth.
+ *   mode SU2_PROBE_COPY: every pass copies the first half onto the second (read + write = `bytes`).
+ * *gbs_out [host] = bytes per pass / mean duration of `passes` passes (CUDA events on cuda_stream, may
+ * be 0), in GB/s (1e9); *us_per_pass_out [host, nullable]. Synchronises that stream.
+ * Errors: SU2_EARG, SU2_EALLOC, SU2_ECUDA. No handle: nothing of a lattice is touched. */
+#define SU2_PROBE_READ 0
+#define SU2_PROBE_COPY 1
+SU2_API int su2_bandwidth_probe(size_t bytes, int passes, int mode, void* cuda_stream, double* gbs_out,
+                                double* us_per_pass_out);
+
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 SU2_API uint64_t su2_launch_count(const su2_lattice* lat);
 

@@ -22,6 +22,7 @@ SU2_START_COLD, SU2_START_HOT = 0, 1
 SU2_DRAW_KP, SU2_DRAW_AUTO, SU2_DRAW_CREUTZ = 0, 1, 2
 SU2_ALPHA_C = 1.6847
 SU2_OPT_OVERLAP, SU2_OPT_RUN_GRAPH = 0, 1
+SU2_PROBE_READ, SU2_PROBE_COPY = 0, 1
 
 _lib = None
 
@@ -66,6 +67,8 @@ _SIGNATURES = {
     "su2_ipc_export": (C.c_int, [C.c_void_p, C.c_void_p]),
     "su2_ipc_open": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p)]),
     "su2_ipc_close": (C.c_int, [C.c_void_p]),
+    "su2_bandwidth_probe": (C.c_int, [C.c_size_t, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_double),
+                                      C.POINTER(C.c_double)]),
     "su2_launch_count": (C.c_uint64, [C.c_void_p]),
     "su2_device_links": (C.c_void_p, [C.c_void_p]),
     "su2_last_error": (C.c_char_p, [C.c_void_p]),
@@ -236,6 +239,13 @@ def su2_set_links(h, host_array):
 
 def su2_synchronize(h):
     _check(lib().su2_synchronize(h), h)
+
+
+def su2_bandwidth_probe(nbytes, passes, mode=SU2_PROBE_READ, cuda_stream=0):
+    """(GB/s, microseconds per pass) of a read or copy pass over a scratch buffer of nbytes."""
+    gbs, us = C.c_double(), C.c_double()
+    _check(lib().su2_bandwidth_probe(nbytes, passes, mode, C.c_void_p(cuda_stream), C.byref(gbs), C.byref(us)))
+    return gbs.value, us.value
 
 
 def su2_launch_count(h):

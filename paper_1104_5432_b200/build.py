@@ -8,7 +8,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsu2hb.so")
-SOURCES = ["su2_heatbath.cu", "su2_measure.cu", "su2_api.cu"]
+SOURCES = ["su2_heatbath.cu", "su2_measure.cu", "su2_probe.cu", "su2_api.cu"]
 HEADERS = ["su2_device.cuh", "su2_launch.h", "su2_math64.cuh", "su2_log_table.inc", os.path.join("..", "..", "include", "su2_heatbath.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]

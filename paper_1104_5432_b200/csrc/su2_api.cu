@@ -782,6 +782,15 @@ extern "C" int su2_ipc_close(void* dev_ptr)
     return SU2_OK;
 }
 
+extern "C" int su2_bandwidth_probe(size_t bytes, int passes, int mode, void* cuda_stream, double* gbs_out,
+                                   double* us_per_pass_out)
+{
+    if (!gbs_out || passes < 1 || passes > 100000 || bytes < (1u << 20) || (bytes & 31) ||
+        (mode != SU2_PROBE_READ && mode != SU2_PROBE_COPY))
+        return SU2_EARG;
+    return run_bandwidth_probe(bytes, passes, mode, (cudaStream_t)cuda_stream, gbs_out, us_per_pass_out);
+}
+
 extern "C" uint64_t su2_launch_count(const su2_lattice* lat) { return lat ? lat->launches : 0; }
 
 extern "C" void* su2_device_links(su2_lattice* lat) { return lat ? lat->links : nullptr; }

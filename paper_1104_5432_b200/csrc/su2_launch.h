@@ -98,4 +98,7 @@ int launch_polyakov_correlator(const Geom& g, const Scratch& sc, int rmax, doubl
 int launch_to_device_layout(const void* canonical, void* links, const Geom& g, int precision, cudaStream_t st);
 int launch_to_canonical(const void* links, void* canonical, const Geom& g, int precision, cudaStream_t st);
 
+// su2_probe.cu: returns an SU2_* code
+int run_bandwidth_probe(size_t bytes, int passes, int mode, cudaStream_t st, double* gbs_out, double* us_per_pass_out);
+
 }  // namespace su2

@@ -68,7 +68,7 @@ def test_sampled_link_parity_at_bench_sizes(dims, prec, start, beta):
                 why = sampled_link_excused(d, mg, k, prec)
                 assert why, (s, mu, d, mg, k)
                 flips += why == "flip"
-                small += why == "small_k"
+                small += why == "conditioned"
         # properties that hold at any size
         mask = np.ones((V, 4), bool)
         mask[par_of(s_all) == p, mu] = False
@@ -77,7 +77,7 @@ def test_sampled_link_parity_at_bench_sizes(dims, prec, start, beta):
         assert np.abs((upd**2).sum(-1) - 1).max() < (9e-16 if prec == 64 else 5e-7)  # 4 ulp on |a|^2
         assert np.abs(after[~mask] - before[~mask]).max() > 1e-3
         del after
-    assert flips <= pp.flip_budget(sampled, prec) and small <= pp.small_k_budget(sampled, prec, haar=False)
+    assert flips <= pp.flip_budget(sampled, prec) and small <= pp.conditioned_budget(sampled, prec, haar=False)
     lat.close()
 
 
@@ -115,10 +115,10 @@ def test_sampled_link_parity_at_32c4_with_auto_draw(prec):
                     why = sampled_link_excused(d, mg, k, prec)
                     assert why, (s, mu, d, mg, k)
                     flips += why == "flip"
-                    small += why == "small_k"
+                    small += why == "conditioned"
             del after
         assert n_creutz > 100 and n_kp > 20      # both branches sampled
-        assert flips <= pp.flip_budget(sampled, prec) and small <= pp.small_k_budget(sampled, prec)
+        assert flips <= pp.flip_budget(sampled, prec) and small <= pp.conditioned_budget(sampled, prec)
         lat.close()
     finally:
         for m in ("f64", "f32", "f32x"):

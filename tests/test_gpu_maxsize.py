@@ -80,7 +80,7 @@ def test_128c3x144_fp32_offsets_beyond_32_bits():
                 why = sampled_link_excused(d, mg, k, prec)
                 assert why, (s, mu, d, mg, k)
                 flips += why == "flip"
-                small += why == "small_k"
+                small += why == "conditioned"
         a6, b6 = after.reshape(nt, nz, ny, nx, 4, 4), before.reshape(nt, nz, ny, nx, 4, 4)
         for nu in range(4):                               # one time slice at a time: bounded temporaries
             for t in range(nt):
@@ -94,7 +94,7 @@ def test_128c3x144_fp32_offsets_beyond_32_bits():
                 assert np.abs((new**2).sum(-1) - 1).max() < 5e-7
                 assert (np.abs(new - b[upd]).max(-1) > 0).mean() > 0.999
         lat.set_links(before)
-    assert flips <= pp.flip_budget(sampled, prec) and small <= pp.small_k_budget(sampled, prec)
+    assert flips <= pp.flip_budget(sampled, prec) and small <= pp.conditioned_budget(sampled, prec)
     lat.close()
 
 

@@ -65,7 +65,7 @@ def test_protocol_verdicts_on_hand_made_deviations():
     m2 = mg.copy()
     m2[s, mu] = 3e-7
     r = pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, m2, kn)
-    assert (r.flips, r.small_k, r.downstream) == (1, 0, 0)
+    assert (r.flips, r.conditioned, r.downstream) == (1, 0, 0)
     # ... two such links exceed the budget of a 2048-link sweep
     gpu2 = gpu.copy()
     gpu2[s + 2, mu] = -gpu2[s + 2, mu]
@@ -95,20 +95,40 @@ def test_protocol_verdicts_on_hand_made_deviations():
         pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, m3, kn)
 
 
-def test_small_k_excuse_scales_with_one_over_k_and_is_fp32_only():
+def test_conditioning_bound_scales_with_one_over_k_and_with_the_inputs_and_is_fp32_only():
     dims = (8, 4, 4, 4)
     ora, mg, kn = _sweep_records(dims, "f32")
+    V = oracle.volume(dims)
     s, mu = 90, 3
     k2 = kn.copy()
-    k2[s, mu] = 0.02                      # E_V / k = 5e-5
+    k2[s, mu] = 0.04                      # E_V / k = 5e-5
     gpu = ora.copy()
     gpu[s, mu, 1] += np.float32(4e-5)
     r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k2)
-    assert (r.flips, r.small_k) == (0, 1)
+    assert (r.flips, r.conditioned) == (0, 1)
     gpu[s, mu, 1] += np.float32(4e-5)     # 8e-5 > E_V / k: more than 1/k explains
     with pytest.raises(AssertionError, match="no excuse"):
         pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k2)
-    # fp64 has no small-k excuse and a zero flip budget
+    # a well-conditioned link (k = 0.5) may exceed 1e-5 only by what the measured deviation of its inputs explains
+    k3 = kn.copy()
+    k3[s, mu] = 0.5
+    gpu = ora.copy()
+    gpu[s, mu, 2] += np.float32(2.5e-5)
+    with pytest.raises(AssertionError, match="no excuse"):
+        pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k3)
+    # ... one of its inputs, updated earlier in the sweep (direction 0), deviates by 8e-6 (inside tolerance):
+    # (E_V + 2 x 8e-6) / 0.5 = 3.6e-5 >= 2.5e-5
+    s_in = s                                             # U_0(x): the staple input 'U_nu(x)' with nu = 0
+    gpu[s_in, 0, 0] += np.float32(8e-6)
+    r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k3)
+    assert (r.flips, r.conditioned, r.downstream) == (0, 1, 0)
+    # the same deviation on a link of direction 3's own sub-step partner (updated later or never read) does not help
+    gpu2 = ora.copy()
+    gpu2[s, mu, 2] += np.float32(2.5e-5)
+    gpu2[(s + 5) % V, 1, 0] += np.float32(8e-6)
+    with pytest.raises(AssertionError, match="no excuse"):
+        pp.compare_links(gpu2, ora, dims, 32, pp.SWEEP, mg, k3)
+    # fp64 has no conditioning excuse and a zero flip budget
     o64, m64, k64 = _sweep_records(dims, "f64")
     g64 = o64.copy()
     g64[s, mu, 1] += 1e-11
@@ -121,10 +141,10 @@ def test_small_k_excuse_scales_with_one_over_k_and_is_fp32_only():
 
 
 def test_budgets():
-    assert pp.flip_budget(65536, 64) == 0 and pp.small_k_budget(65536, 64) == 0
+    assert pp.flip_budget(65536, 64) == 0 and pp.conditioned_budget(65536, 64) == 0
     assert pp.flip_budget(16, 32) == 1 and pp.flip_budget(65536, 32) == 1
     assert pp.flip_budget(4 * 32**4, 32) == int(np.ceil(5 * pp.FLIP_RATE[32] * 4 * 32**4))
-    assert pp.small_k_budget(65536, 32) == 2 and pp.small_k_budget(65536, 32, haar=False) == 1
+    assert pp.conditioned_budget(65536, 32) == 7 and pp.conditioned_budget(65536, 32, haar=False) == 1
 
 
 def test_fp32_oracle_modes_agree_under_the_protocol():
