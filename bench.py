@@ -460,6 +460,60 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------- roofline
+def load_traffic():
+    """profiles/traffic.csv: key,bytes_per_launch,source - dram__bytes_read.sum + dram__bytes_write.sum per
+    heat-bath launch from the committed `ncu --set full` captures (a citation, not a quantity of this run)"""
+    out = {}
+    prof = os.path.join(ROOT, "profiles", "traffic.csv")
+    if os.path.exists(prof):
+        with open(prof) as f:
+            for row in f:
+                k = row.strip().split(",")
+                if len(k) >= 2 and not k[0].startswith("#"):
+                    try:
+                        out[k[0]] = (float(k[1]), k[2] if len(k) > 2 else "profiles/")
+                    except ValueError:
+                        pass
+    return out
+
+
+def roofline_point(w, prec, r, hbm_peak, hbm_src, l2_gbs, traffic, sampler):
+    """Roofline of the dominant kernel (heat-bath sub-step) at one point of the metric. Algorithmic bytes per
+    launch = (V/2 updates) x 8 quaternions; duration = mean time of the 8 sub-steps of a
+    sweep / 8, CUDA events on the launching stream inside the timed region; burst (`frac`) and sustained
+    (`frac_sustained`, >= 1 s of continuous steps) legs. A lattice that fits the 126 MB L2 is bound by the L2
+    bandwidth of the box (measured by su2_bandwidth_probe in this run) and is quoted against it; its
+    fraction of the HBM copy peak is kept beside it for comparison with the other points."""
+    alg = (w.volume // 2) * BYTES_PER_UPDATE[prec]
+    lattice_mib = w.links * 4 * prec // 8 >> 20
+    resident = lattice_mib <= 100 and l2_gbs is not None
+    peak = l2_gbs if resident else hbm_peak
+    sub_us = r["sweep_ms"] * 1e3 / 8.0
+    ach = alg / (sub_us * 1e-6) / 1e9
+    key = f"{w.name}_fp{prec}"
+    pt = {"bound": "l2" if resident else "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+          "traffic": traffic.get(key, (None, None))[0],
+          "traffic_kind": "ncu --set full capture committed under profiles/ (not measured in this run): "
+                          + str(traffic.get(key, (None, "none for this point"))[1]),
+          "peak_source": ("measured in this run: su2_bandwidth_probe, 64 MiB read, L2-resident (lattice %d MiB)" % lattice_mib)
+          if resident else hbm_src,
+          "algorithmic_bytes_per_launch": alg, "avg_launch_us": sub_us,
+          "frac_of_hbm_peak": ach / hbm_peak, "steps": int(round(r["ms_total"] / r["ms_per_step"])),
+          "ms_per_step": r["ms_per_step"], "clocks": sampler.summary(*r["t_wall"]) if sampler else None}
+    if "sustained" in r:
+        su = r["sustained"]
+        sus_us = su["sweep_ms"] * 1e3 / 8.0
+        a2 = alg / (sus_us * 1e-6) / 1e9
+        pt.update({"frac_sustained": a2 / peak, "achieved_sustained": a2, "avg_launch_us_sustained": sus_us,
+                   "sustained_region_ms": su["ms_total"], "sustained_steps": su["steps"],
+                   "sustained_ms_per_step": su["ms_per_step"], "frac_of_hbm_peak_sustained": a2 / hbm_peak,
+                   "clocks_sustained": sampler.summary(*su["t_wall"]) if sampler else None})
+    if l2_gbs is not None:
+        pt["l2_read_gbs_measured"] = l2_gbs
+    return pt
+
+
 # ------------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -475,6 +529,10 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-seconds", type=float, default=120.0, help="host time the whole reference run may take")
     ap.add_argument("--cpu-baseline-seconds", type=float, default=12.0)
+    ap.add_argument("--sustained-seconds", type=float, default=1.0,
+                    help="length of the sustained (power-capped) timed region per metric point; 0 = skip")
+    ap.add_argument("--split", default="replicas", choices=["replicas", "slabs"],
+                    help="--gpus N > 1: independent replicas (default, north_star) or ONE lattice as N time slabs")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -505,7 +563,8 @@ def main():
     t_wait = time.time()
     while not sampler.ready() and time.time() - t_wait < 5.0:  # nvidia-smi takes ~1 s to emit its first line
         time.sleep(0.05)
-    r = time_workload(pkg, torch, w, prec, args.beta, args.steps, args.warmup, args.seed + rank, sampler, dist)
+    sus_s = 0.0 if args.headline_only else args.sustained_seconds
+    r = time_workload(pkg, torch, w, prec, args.beta, args.steps, args.warmup, args.seed + rank, sampler, dist, sus_s)
     clocks = sampler.summary(*r["t_wall"])
 
     ms = r["ms_total"]
@@ -515,28 +574,19 @@ def main():
         ms = float(t.item())
     value = world * w.links * args.steps / (ms * 1e-3)
 
-    # roofline of the dominant kernel (heat-bath sub-step): algorithmic bytes per launch =
-    # (V/2 updates) * 8 quaternions; duration = sweep time / 8 launches, CUDA events on the
-    # launching stream inside the timed region.
-    sub_s = r["sweep_ms"] * 1e-3 / 8.0
-    alg_bytes = (w.volume // 2) * BYTES_PER_UPDATE[prec]
-    achieved = alg_bytes / sub_s / 1e9
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "kernel": "heatbath sub-step (one per (mu,parity))",
-                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_us": sub_s * 1e6}
-    # traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of that kernel from the
-    # committed `ncu --set full` capture (profiles/traffic.csv: key,bytes_per_launch,source)
-    prof = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(prof):
-        try:
-            with open(prof) as f:
-                for row in f:
-                    k = row.strip().split(",")
-                    if k and k[0] == f"{w.name}_fp{prec}":
-                        roofline["traffic"] = float(k[1])
-                        roofline["traffic_source"] = k[2] if len(k) > 2 else "profiles/"
-        except Exception:
-            pass
+    # L2 roofline denominator: read bandwidth of a 64 MiB buffer - the size of the
+    # 32^4 fp32 lattice - once it is resident in the 126 MB L2; measured live by the library's probe kernel
+    l2_gbs = None
+    if rank == 0 and not args.headline_only:
+        time.sleep(COOL_DOWN_S)
+        l2_gbs, _ = pkg.su2_bandwidth_probe(64 << 20, 400, pkg.SU2_PROBE_READ)
+
+    traffic = load_traffic()
+    point = lambda name, p, rr: roofline_point(workloads.BY_NAME[name], p, rr, peak, peak_src, l2_gbs, traffic, sampler)
+    head_key = f"{w.name}_fp{prec}"
+    roofline = point(w.name, prec, r)
+    roofline["kernel"] = "heatbath sub-step (one launch per (mu, parity), 8 per sweep)"
+    roofline["points"] = {head_key: {k: v for k, v in roofline.items() if k != "kernel"}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -559,24 +609,19 @@ def main():
     }
 
     if not args.headline_only and rank == 0:
-        # the other points of the metric, device-resident, same step
+        # the other three points of the metric (fp32/fp64 at 32^4 and 64^4), device-resident, same step, each
+        # with its burst and sustained fraction inside `roofline.points`
         others = {}
-        for name, p in (("C5_64^4", 64), ("C3_32^4", 32), ("C3_32^4", 64)):
+        for name, p in (("C5_64^4", 32), ("C5_64^4", 64), ("C3_32^4", 32), ("C3_32^4", 64)):
             if name == w.name and p == prec:
                 continue
             ww = workloads.BY_NAME[name]
-            rr = time_workload(pkg, torch, ww, p, args.beta, args.steps, args.warmup, args.seed)
-            ss = rr["sweep_ms"] * 1e-3 / 8.0
-            ach = (ww.volume // 2) * BYTES_PER_UPDATE[p] / ss / 1e9
-            lattice_mib = ww.links * 4 * p // 8 >> 20
+            rr = time_workload(pkg, torch, ww, p, args.beta, args.steps, args.warmup, args.seed, sampler, None, sus_s)
+            roofline["points"][f"{name}_fp{p}"] = point(name, p, rr)
             others[f"{name}_fp{p}"] = {
                 "value": ww.links * args.steps / (rr["ms_total"] * 1e-3), "unit": UNIT,
                 "ms_per_step": rr["ms_per_step"], "ms_per_sweep": rr["sweep_ms"],
-                "roofline_frac_hbm": ach / peak, "achieved_gbs": ach,
-                "note": ("lattice %d MiB: L2-resident, HBM peak is not its bound" % lattice_mib) if lattice_mib <= 126
-                else ("lattice %d MiB > L2" % lattice_mib),
-                "plaquette_last": rr["plaquette_last"],
-                "su2_run_ms_per_step": rr["ms_per_step_run"],
+                "plaquette_last": rr["plaquette_last"], "su2_run_ms_per_step": rr["ms_per_step_run"],
             }
         line["workloads"] = others
         line["aux"] = time_aux(pkg, torch, workloads)

@@ -120,8 +120,7 @@ __device__ __forceinline__ Quat<double> ldq(const double4a* p)
 #ifndef HB_ST
 #define HB_ST ".cs"
 #endif
-// L2-only loads (no L1 allocation): used for the links the preceding sub-step wrote,
-// which are read after griddepcontrol.wait while that kernel may still share the SM.
+// L2-only loads (no L1 allocation): streams that are read once (the Polyakov lines).
 __device__ __forceinline__ Quat<float> ldq_cg(const float4* p)
 {
     Quat<float> q;
@@ -135,6 +134,34 @@ __device__ __forceinline__ Quat<double> ldq_cg(const double4a* p)
 {
     Quat<double> q;
     asm volatile("ld.global.cg.v4.f64 {%0,%1,%2,%3}, [%4];"
+                 : "=d"(q.a0), "=d"(q.a1), "=d"(q.a2), "=d"(q.a3)
+                 : "l"(p)
+                 : "memory");
+    return q;
+}
+// Loads of the links the PRECEDING sub-step wrote, issued after griddepcontrol.wait: ordinary
+// (coherent, L1-allocating) ld.global, not the read-only .nc path - the array was written while this kernel's
+// CTAs were already being scheduled. An ordinary load after the wait observes the primary grid's flushed
+// writes; no earlier kernel's copy can linger in L1, which is invalidated at every launch, and the kernel
+// launched in between never reads that array. U_mu on the other parity is the most re-used operand of a tile
+// (6 reads per link): through L2 only (.cg, round 1) these loads cost 14 % more L2 -> SM traffic per launch
+// (ncu: 2.24 against 1.93 GB at 64^4 fp32, profiles/r02b.md).
+#ifndef HB_DEP_LD
+#define HB_DEP_LD ""
+#endif
+__device__ __forceinline__ Quat<float> ldq_dep(const float4* p)
+{
+    Quat<float> q;
+    asm volatile("ld.global" HB_DEP_LD ".v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(q.a0), "=f"(q.a1), "=f"(q.a2), "=f"(q.a3)
+                 : "l"(p)
+                 : "memory");
+    return q;
+}
+__device__ __forceinline__ Quat<double> ldq_dep(const double4a* p)
+{
+    Quat<double> q;
+    asm volatile("ld.global" HB_DEP_LD ".v4.f64 {%0,%1,%2,%3}, [%4];"
                  : "=d"(q.a0), "=d"(q.a1), "=d"(q.a2), "=d"(q.a3)
                  : "l"(p)
                  : "memory");
@@ -445,22 +472,9 @@ __device__ __forceinline__ double block_sum(double v, double* red)
     return tot;
 }
 
-// Same, for a per-thread value of the lattice precision: in fp32 the 32 lanes are summed in
-// fp32 (5 shuffles instead of 10; the warp sum of <= 192 is good to ~1e-7 relative, far
-// inside the 1e-6 plaquette tolerance), the 4-8 warp sums and everything after in fp64.
-// No trailing barrier: for one use at the end of a kernel.
-__device__ __forceinline__ double block_sum_end(float v, double* red)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-    if (lane == 0) red[wid] = (double)v;
-    __syncthreads();
-    double tot = 0.0;
-    if (threadIdx.x == 0)
-        for (int i = 0; i < nw; ++i) tot += red[i];
-    return tot;
-}
+// Same without the trailing barrier: for one use at the end of a kernel. The per-thread value is converted
+// to fp64 BEFORE the first shuffle (north_star: reductions "accumulated in fp64"; round 1 summed the 32 lanes
+// of an fp32 kernel in fp32 - 5 shuffles fewer in 3 of the 8 kernels of a sweep, not measurable).
 __device__ __forceinline__ double block_sum_end(double v, double* red)
 {
 #pragma unroll

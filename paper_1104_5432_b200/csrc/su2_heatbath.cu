@@ -94,6 +94,10 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     const Nbr d = neighbours(g, c, ix.r);
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
     const uint32_t h_up = HB_CK(h + d.up[MU]);
+#ifndef HB_ORDER
+#define HB_ORDER 0
+#endif
+#if HB_ORDER == 0
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         const int nu = i + (i >= MU ? 1 : 0);
@@ -101,16 +105,87 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
         const L* o_nu = hp.oppo[nu];
         const uint32_t h_dn = HB_CK(h + d.dn[nu]);
         const uint32_t h_upnu = HB_CK(h + d.up[nu]);
-        q.a[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
-        q.b[i] = DEP_MU ? ldq_cg(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
+        q.a[i] = (nu == DEP_NU) ? ldq_dep(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
+        q.b[i] = DEP_MU ? ldq_dep(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
         q.cc[i] = ldq(s_nu + HB_CK(h));                                      // U_nu(x)
         q.a2[i] = ldq(s_nu + HB_CK((int)h_up + d.dn[nu]));               // U_nu(x+mu-nu)
-        q.b2[i] = DEP_MU ? ldq_cg(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
-        q.c2[i] = (nu == DEP_NU) ? ldq_cg(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
+        q.b2[i] = DEP_MU ? ldq_dep(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
+        q.c2[i] = (nu == DEP_NU) ? ldq_dep(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
         // su2_run's loop state is fetched behind the first six link loads: its round trip then
         // overlaps theirs instead of preceding them (the n = 0 Philox call needs `sweep`)
         if (i == 0) run_state(hp, sweep, inv_beta);
     }
+#elif HB_ORDER == 3
+    // First-touch loads first. CTAs sweep the lattice x fastest, then y, z, t; of the reads of one array in a
+    // sub-step the one that reaches furthest ahead in that order misses L2, the others find the line the
+    // earlier CTA brought in: U_nu(x+mu) is always ahead of U_nu(x-nu); U_nu(x+mu-nu) is ahead of U_nu(x)
+    // iff mu > nu; of the six reads of U_mu the one at x+nu with the largest nu. Those 7 go out as the first
+    // batch, so that the later batches wait for cache hits only.
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const int nu = i + (i >= MU ? 1 : 0);
+        q.a[i] = (nu == DEP_NU) ? ldq_dep(hp.oppo[nu] + h_up) : ldq(hp.oppo[nu] + h_up);  // U_nu(x+mu)
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const int nu = i + (i >= MU ? 1 : 0);
+        if (MU > nu) q.a2[i] = ldq(hp.same[nu] + HB_CK((int)h_up + d.dn[nu]));  // U_nu(x+mu-nu)
+        else q.cc[i] = ldq(hp.same[nu] + HB_CK(h));                             // U_nu(x)
+    }
+    {
+        constexpr int nu = (MU == 3) ? 2 : 3;
+        const uint32_t h_upnu = HB_CK(h + d.up[nu]);
+        q.b[2] = DEP_MU ? ldq_dep(o_mu + h_upnu) : ldq(o_mu + h_upnu);  // U_mu(x+nu), largest nu
+    }
+    run_state(hp, sweep, inv_beta);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const int nu = i + (i >= MU ? 1 : 0);
+        const uint32_t h_dn = HB_CK(h + d.dn[nu]);
+        if (i < 2) {
+            const uint32_t h_upnu = HB_CK(h + d.up[nu]);
+            q.b[i] = DEP_MU ? ldq_dep(o_mu + h_upnu) : ldq(o_mu + h_upnu);  // U_mu(x+nu)
+        }
+        if (MU > nu) q.cc[i] = ldq(hp.same[nu] + HB_CK(h));
+        else q.a2[i] = ldq(hp.same[nu] + HB_CK((int)h_up + d.dn[nu]));
+        q.b2[i] = DEP_MU ? ldq_dep(o_mu + h_dn) : ldq(o_mu + h_dn);                         // U_mu(x-nu)
+        q.c2[i] = (nu == DEP_NU) ? ldq_dep(hp.oppo[nu] + h_dn) : ldq(hp.oppo[nu] + h_dn);  // U_nu(x-nu)
+    }
+#else
+    // forward loads first: U_nu(x+mu) and U_nu(x+mu-nu) reach ahead of the CTA sweep through the lattice and are
+    // the ones that miss L2; issued as the first batch, the later batches only wait for cache hits
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const int nu = i + (i >= MU ? 1 : 0);
+        q.a[i] = (nu == DEP_NU) ? ldq_dep(hp.oppo[nu] + h_up) : ldq(hp.oppo[nu] + h_up);  // U_nu(x+mu)
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const int nu = i + (i >= MU ? 1 : 0);
+        q.a2[i] = ldq(hp.same[nu] + HB_CK((int)h_up + d.dn[nu]));  // U_nu(x+mu-nu)
+    }
+#if HB_ORDER == 2
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const int nu = i + (i >= MU ? 1 : 0);
+        const uint32_t h_upnu = HB_CK(h + d.up[nu]);
+        q.b[i] = DEP_MU ? ldq_dep(o_mu + h_upnu) : ldq(o_mu + h_upnu);  // U_mu(x+nu)
+    }
+#endif
+    run_state(hp, sweep, inv_beta);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const int nu = i + (i >= MU ? 1 : 0);
+        const uint32_t h_dn = HB_CK(h + d.dn[nu]);
+#if HB_ORDER != 2
+        const uint32_t h_upnu = HB_CK(h + d.up[nu]);
+        q.b[i] = DEP_MU ? ldq_dep(o_mu + h_upnu) : ldq(o_mu + h_upnu);  // U_mu(x+nu)
+#endif
+        q.cc[i] = ldq(hp.same[nu] + HB_CK(h));                                            // U_nu(x)
+        q.b2[i] = DEP_MU ? ldq_dep(o_mu + h_dn) : ldq(o_mu + h_dn);                        // U_mu(x-nu)
+        q.c2[i] = (nu == DEP_NU) ? ldq_dep(hp.oppo[nu] + h_dn) : ldq(hp.oppo[nu] + h_dn);  // U_nu(x-nu)
+    }
+#endif
     return ix;
 }
 
@@ -251,7 +326,7 @@ struct MinBlocks<double> {
 // tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile;
 // grid = (nb0, nb1, nb2*nb3): x fastest, so CTAs are scheduled roughly in memory order.
 template <typename Real, int MU, int P, bool MEAS, bool ALT, int LHX, int LY, int LZ, int LT>
-__global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::value)
+__global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), (MinBlocks<Real>::value << 7) >> (LHX + LY + LZ + LT))
     heatbath_tiled_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
     uint32_t rep = 0, bzt = blockIdx.z;
@@ -261,10 +336,34 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), MinBlocks<Real>::va
     }
     Site c = tile_site<LHX, LY, LZ, LT>(g, bzt);
     if (ALT) c.t += g.t_lo;  // slab: the grid covers the interior slices only
+#ifdef HB_PF
+    // L2 prefetch (TMA unit) of the forward rows of the tile HB_PF z-t tile rows ahead in dispatch order:
+    // thread j < 6 * rows: array j / rows (three nu, both parities) at x+mu, row j % rows of that tile
+    if (!ALT) {
+        constexpr int ROWS = 1 << (LY + LZ + LT);
+        const int j = threadIdx.x;
+        const uint32_t bzt2 = bzt + HB_PF;
+        if (j < 6 * ROWS && bzt2 < (uint32_t)(g.nb[2] * g.nb[3])) {
+            const uint32_t bt2 = (g.nb[2] == 1) ? bzt2 : __umulhi(bzt2, g.zmagic);
+            const uint32_t bz2 = bzt2 - bt2 * (uint32_t)g.nb[2];
+            const int row = j & (ROWS - 1), a = j >> (LY + LZ + LT);  // a = 0..5
+            const int i = a >> 1, nu = i + (i >= MU ? 1 : 0);
+            int y = (int)(blockIdx.y << LY) + (row & ((1 << LY) - 1));
+            int z = (int)(bz2 << LZ) + ((row >> LY) & ((1 << LZ) - 1));
+            int t = (int)(bt2 << LT) + (row >> (LY + LZ));
+            if (MU == 1) y = (y + 1 == g.n[1]) ? 0 : y + 1;
+            if (MU == 2) z = (z + 1 == g.n[2]) ? 0 : z + 1;
+            if (MU == 3) t = (t + 1 == g.n[3]) ? 0 : t + 1;
+            const int h0 = (int)(blockIdx.x << LHX) + g.sy * y + g.sz * z + g.st * t;
+            const typename LinkPtr<Real>::type* src = ((a & 1) ? hp.same[nu] : hp.oppo[nu]) + h0;
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)(sizeof(*src) << LHX)) : "memory");
+        }
+    }
+#endif
     const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err);
     if (MEAS) {  // one fp64 partial per CTA, fixed order
         __shared__ double red[kBlock / 32];
-        const double tot = block_sum_end(e, red);
+        const double tot = block_sum_end((double)e, red);
         if (threadIdx.x == 0)
             hp.epart[(size_t)rep * hp.epart_stride + blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * bzt)] = tot;
     }
@@ -290,7 +389,7 @@ __global__ void __launch_bounds__(kBlock)
     }
     if (MEAS) {
         __shared__ double red[kBlock / 32];
-        const double tot = block_sum_end(e, red);
+        const double tot = block_sum_end((double)e, red);
         if (threadIdx.x == 0) hp.epart[(size_t)blockIdx.y * hp.epart_stride + blockIdx.x] = tot;
     }
 }
