@@ -460,6 +460,52 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------- one lattice over N GPUs
+def run_slabs(args, torch, pkg, workloads, dist, rank, world, local):
+    """--gpus N --split slabs: ONE lattice as N time slabs, one rank per GPU - the paper's second mode
+    ("2 GPUs"). Each sub-step's kernel also stores the slab's edge slices
+    into the neighbours' halos over NVLink (CUDA-IPC-mapped peer buffers, no pack/send/unpack), a 1-element
+    NCCL all-reduce on the kernels' stream is the barrier between sub-steps. A step = sweep (plaquette
+    fused) + plaquette sum over ranks + chained Polyakov loop. Total work is fixed: strong scaling.
+    Off by default: north_star's metric is single-GPU and --gpus N runs replicas."""
+    from paper_1104_5432_b200 import slabs
+    w = workloads.BY_NAME[args.workload]
+    prec = args.precision
+    ds = slabs.DistributedSlab(w.dims, prec, f"cuda:{local}", barrier="stream")
+    ds.init(w.start, args.seed)
+    P = L = 0.0
+    for i in range(args.warmup):
+        ds.sweep(args.beta, i, fuse_plaquette=True)
+        P, L = ds.mean_plaquette(fused=True), ds.polyakov_loop()
+    dist.barrier()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for k in range(args.steps):
+        ds.sweep(args.beta, args.warmup + k, fuse_plaquette=True)
+        P, L = ds.mean_plaquette(fused=True), ds.polyakov_loop()
+    b.record()
+    torch.cuda.synchronize()
+    dist.barrier()
+    t = torch.tensor([a.elapsed_time(b)], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    ds.close()
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": w.links * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
+            "config": {"workload": f"{w.name} beta={args.beta} start={w.start} seed={args.seed}", "precision": prec,
+                       "parallelism": f"time slabs: one lattice split along t over {world} GPUs, halo links stored "
+                                      "into peer memory by the sub-step kernel, NCCL stream barrier per sub-step",
+                       "l2": "inputs larger than L2, no flush needed"},
+            "gpu_launches": 8 * args.steps + 2 * args.steps, "plaquette_last": P, "polyakov_last": L,
+            "roofline": None, "e2e": None,
+            "note": "opt-in arm (--split slabs); the headline metric and its roofline are the single-GPU run"}))
+    return 0
+
+
 # ------------------------------------------------------------------------------- roofline
 def load_traffic():
     """profiles/traffic.csv: key,bytes_per_launch,source - dram__bytes_read.sum + dram__bytes_write.sum per
@@ -554,6 +600,10 @@ def main():
     from paper_1104_5432_b200 import build as lib_build
     lib_build.build()  # no-op unless a source is newer than the in-tree library
     pkg.lib()
+    if world > 1 and args.split == "slabs":
+        rc = run_slabs(args, torch, pkg, workloads, dist, rank, world, local)
+        dist.destroy_process_group()
+        return rc
     peak, peak_src = measured_peaks()
     w = workloads.BY_NAME[args.workload]
     prec = args.precision

@@ -95,7 +95,7 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
     const uint32_t h_up = HB_CK(h + d.up[MU]);
 #ifndef HB_ORDER
-#define HB_ORDER 0
+#define HB_ORDER 3
 #endif
 #if HB_ORDER == 0
 #pragma unroll

@@ -56,41 +56,32 @@ __global__ void __launch_bounds__(kBlock)
     if (threadIdx.x == 0) partials[blockIdx.y * gridDim.x + blockIdx.x] = tot;
 }
 
-// Tiled form: one CTA = the heat-bath tile of BOTH parities (threads 0..T-1 the even sites,
-// T..2T-1 the odd ones). Every link of the tile is read four times - once as U_mu(x) of its own site and
-// three times as a forward neighbour of the other parity - and with both parities in one CTA three of the
-// four reads are served by L1 instead of L2 (the kernel was bound by L2 -> SM traffic, 16 quaternions per
-// site against 4 compulsory: profiles/r02b.md). The 8 array bases come resolved from the host and element
-// indices are 32-bit (one IMAD.WIDE per load); all 16 links of a site are requested before the first
-// product; the six plaquettes of a site are summed in the lattice precision and enter the fp64
-// accumulation once (fp32: 6 terms of magnitude <= 1, rounding <= 4e-7 per site, random in sign). One
-// partial per CTA, indexed by the linear CTA id.
+// Tiled form (same CTA tiles as the heat-bath kernel): grid.x carries
+// (tile along x, parity), parity fastest, so the two CTAs that read the same 8 tiles of
+// links are scheduled back to back and the second is served by L2 (with parity slowest
+// ncu showed 2.15 GB of DRAM reads for 1.07 GB of links). All 16 links of a site are requested before the
+// first product; one partial per CTA, indexed by the linear CTA id.
+// Measured and rejected in round 2 (profiles/r02b.md): both parities of a tile in ONE 256-thread CTA (L1 then
+// serves 56 % of the reads, L2 -> SM traffic falls by 30 %, yet 347 against 302 us at 64^4 fp32), and host-resolved
+// array bases with 32-bit indices and an fp32 per-site sum (11 % fewer instructions, 343 us): the kernel is
+// bound by the latency of its load batches at 29 resident warps, neither by L2 bandwidth nor by issue slots.
 #ifndef PLAQ_MINB_F32
 #define PLAQ_MINB_F32 8
 #endif
 #ifndef PLAQ_MINB_F64
 #define PLAQ_MINB_F64 4
 #endif
-template <typename Real>
-struct __align__(16) PlaqParams {
-    const typename LinkPtr<Real>::type* arr[2][4];  // [parity][mu]
-};
 template <typename Real, int LHX, int LY, int LZ, int LT>
-__global__ void __launch_bounds__(2 << (LHX + LY + LZ + LT),
-                                  ((sizeof(Real) == 4 ? PLAQ_MINB_F32 : PLAQ_MINB_F64) << 6) >> (LHX + LY + LZ + LT))
-    plaquette_tiled_kernel(const PlaqParams<Real> pp, const Geom g, double* __restrict__ partials)
+__global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT),
+                                  ((sizeof(Real) == 4 ? PLAQ_MINB_F32 : PLAQ_MINB_F64) << 7) >> (LHX + LY + LZ + LT))
+    plaquette_tiled_kernel(const typename LinkPtr<Real>::type* __restrict__ links, const Geom g,
+                           double* __restrict__ partials)
 {
-    constexpr int T = 1 << (LHX + LY + LZ + LT);
-    __shared__ double red[2 * T / 32];
-    const int p = threadIdx.x >> (LHX + LY + LZ + LT);  // warp-uniform
-    const int tid = threadIdx.x & (T - 1);
-    const uint32_t bt = (g.nb[2] == 1) ? blockIdx.z : __umulhi(blockIdx.z, g.zmagic);
-    const uint32_t bz = blockIdx.z - bt * (uint32_t)g.nb[2];
-    Site c;
-    c.hx = (int)(blockIdx.x << LHX) + (tid & ((1 << LHX) - 1));
-    c.y = (int)(blockIdx.y << LY) + ((tid >> LHX) & ((1 << LY) - 1));
-    c.z = (int)(bz << LZ) + ((tid >> (LHX + LY)) & ((1 << LZ) - 1));
-    c.t = (int)(bt << LT) + (tid >> (LHX + LY + LZ)) + g.t_lo;  // slab: interior slices only (t_lo = 0 otherwise)
+    typedef typename LinkPtr<Real>::type L;
+    __shared__ double red[kBlock / 32];
+    const int p = blockIdx.x & 1;
+    Site c = tile_site<LHX, LY, LZ, LT>(g, blockIdx.z, blockIdx.x >> 1);
+    c.t += g.t_lo;  // slab: interior slices only (0 for a whole lattice)
     const int r = (c.y + c.z + c.t + p) & 1;
     const int h = c.hx + g.sy * c.y + g.sz * c.z + g.st * c.t;
     int up[4];
@@ -98,29 +89,32 @@ __global__ void __launch_bounds__(2 << (LHX + LY + LZ + LT),
     up[1] = (c.y + 1 == g.n[1]) ? g.wup[1] : g.sy;
     up[2] = (c.z + 1 == g.n[2]) ? g.wup[2] : g.sz;
     up[3] = (c.t + 1 == g.n[3]) ? g.wup[3] : g.st;
+    const size_t vh = g.vh;
+    const L* same = links + (size_t)(p * 4) * vh;
+    const L* oppo = links + (size_t)((1 - p) * 4) * vh;
     Quat<Real> u[4], n1[6], n2[6];
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) u[mu] = ldq(pp.arr[p][mu] + (uint32_t)h);
+    for (int mu = 0; mu < 4; ++mu) u[mu] = ldq(same + mu * vh + (uint32_t)h);
     {
         int k = 0;
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu)
 #pragma unroll
             for (int nu = mu + 1; nu < 4; ++nu, ++k) {
-                n1[k] = ldq(pp.arr[1 - p][nu] + (uint32_t)(h + up[mu]));  // U_nu(x+mu)
-                n2[k] = ldq(pp.arr[1 - p][mu] + (uint32_t)(h + up[nu]));  // U_mu(x+nu)
+                n1[k] = ldq(oppo + nu * vh + (uint32_t)(h + up[mu]));  // U_nu(x+mu)
+                n2[k] = ldq(oppo + mu * vh + (uint32_t)(h + up[nu]));  // U_mu(x+nu)
             }
     }
-    Real site = 0;
+    double acc = 0.0;
     {
         int k = 0;
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu)
 #pragma unroll
             for (int nu = mu + 1; nu < 4; ++nu, ++k)
-                site += qdot(qmul<false, false>(u[mu], n1[k]), qmul<false, false>(u[nu], n2[k]));
+                acc += (double)qdot(qmul<false, false>(u[mu], n1[k]), qmul<false, false>(u[nu], n2[k]));
     }
-    const double tot = block_sum((double)site, red);
+    const double tot = block_sum(acc, red);
     if (threadIdx.x == 0) partials[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = tot;
 }
 
@@ -419,17 +413,16 @@ static void launch_plaquette_t(const void* links, const Geom& g, const Scratch& 
 {
     typedef typename LinkPtr<Real>::type L;
     if (g.tile >= 0) {
-        const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
+        const dim3 grid(2u * (unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3]));
         *n_partials = (size_t)grid.x * grid.y * grid.z;
-        PlaqParams<Real> pp;
-        for (int p = 0; p < 2; ++p)
-            for (int mu = 0; mu < 4; ++mu) pp.arr[p][mu] = (const L*)links + (size_t)(p * 4 + mu) * g.vh;
         if (g.tile == 0)
             plaquette_tiled_kernel<Real, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>
-                <<<grid, 2 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3]), 0, st>>>(pp, g, sc.partials);
+                <<<grid, 1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3]), 0, st>>>((const L*)links, g,
+                                                                                                    sc.partials);
         else
             plaquette_tiled_kernel<Real, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3]>
-                <<<grid, 2 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3]), 0, st>>>(pp, g, sc.partials);
+                <<<grid, 1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3]), 0, st>>>((const L*)links, g,
+                                                                                                    sc.partials);
     } else {
         const dim3 grid(blocks_for((uint64_t)g.st * g.nt_upd), 2);
         *n_partials = (size_t)grid.x * 2;
