@@ -146,7 +146,7 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, int nrep, 
     g.wup[3] = -(Nt - 1) * g.st;
     g.t_lo = slab_Lt > 0 ? 2 : 0;
     g.nt_upd = slab_Lt > 0 ? slab_Lt : Nt;
-    choose_tiling(g, nrep);  // grid z holds (replica, z-t tile): falls back to the next shape / the linear launch
+    choose_tiling(g, nrep, precision);  // grid z holds (replica, z-t tile): falls back to the next shape / the linear launch
     lat->nrep = nrep;
     lat->rep_bytes = rep_bytes;
     lat->precision = precision;

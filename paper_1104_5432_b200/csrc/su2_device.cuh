@@ -24,6 +24,7 @@ struct Geom {
     int nb[4];       // tiled launch: number of tiles along hx, y, z, t
     int wup[4];      // half-index delta of +mu at the upper boundary: -(N-1)*stride  (x: -(nxh-1))
     uint32_t zmagic; // ceil(2^32 / nb[2]): blockIdx.z -> (bz, bt) without a division
+    int tloop;       // heat-bath tiled launch: consecutive t-tiles one CTA walks through (divides nb[3])
     // time slab of a lattice split over GPUs: only the slices t_lo <= t < t_lo + nt_upd
     // are updated and measured, the others are halo copies. Whole lattice: t_lo = 0, nt_upd = Nt.
     int t_lo, nt_upd;
@@ -146,13 +147,10 @@ __device__ __forceinline__ Quat<double> ldq_cg(const double4a* p)
 // launched in between never reads that array. U_mu on the other parity is the most re-used operand of a tile
 // (6 reads per link): through L2 only (.cg, round 1) these loads cost 14 % more L2 -> SM traffic per launch
 // (ncu: 2.24 against 1.93 GB at 64^4 fp32, profiles/r02b.md).
-#ifndef HB_DEP_LD
-#define HB_DEP_LD ""
-#endif
 __device__ __forceinline__ Quat<float> ldq_dep(const float4* p)
 {
     Quat<float> q;
-    asm volatile("ld.global" HB_DEP_LD ".v4.f32 {%0,%1,%2,%3}, [%4];"
+    asm volatile("ld.global.v4.f32 {%0,%1,%2,%3}, [%4];"
                  : "=f"(q.a0), "=f"(q.a1), "=f"(q.a2), "=f"(q.a3)
                  : "l"(p)
                  : "memory");
@@ -161,7 +159,7 @@ __device__ __forceinline__ Quat<float> ldq_dep(const float4* p)
 __device__ __forceinline__ Quat<double> ldq_dep(const double4a* p)
 {
     Quat<double> q;
-    asm volatile("ld.global" HB_DEP_LD ".v4.f64 {%0,%1,%2,%3}, [%4];"
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];"
                  : "=d"(q.a0), "=d"(q.a1), "=d"(q.a2), "=d"(q.a3)
                  : "l"(p)
                  : "memory");

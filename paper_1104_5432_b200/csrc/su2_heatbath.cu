@@ -94,28 +94,6 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
     const Nbr d = neighbours(g, c, ix.r);
     const L* o_mu = hp.oppo[MU];  // U_mu on the other parity
     const uint32_t h_up = HB_CK(h + d.up[MU]);
-#ifndef HB_ORDER
-#define HB_ORDER 3
-#endif
-#if HB_ORDER == 0
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        const int nu = i + (i >= MU ? 1 : 0);
-        const L* s_nu = hp.same[nu];
-        const L* o_nu = hp.oppo[nu];
-        const uint32_t h_dn = HB_CK(h + d.dn[nu]);
-        const uint32_t h_upnu = HB_CK(h + d.up[nu]);
-        q.a[i] = (nu == DEP_NU) ? ldq_dep(o_nu + h_up) : ldq(o_nu + h_up);   // U_nu(x+mu)
-        q.b[i] = DEP_MU ? ldq_dep(o_mu + h_upnu) : ldq(o_mu + h_upnu);       // U_mu(x+nu)
-        q.cc[i] = ldq(s_nu + HB_CK(h));                                      // U_nu(x)
-        q.a2[i] = ldq(s_nu + HB_CK((int)h_up + d.dn[nu]));               // U_nu(x+mu-nu)
-        q.b2[i] = DEP_MU ? ldq_dep(o_mu + h_dn) : ldq(o_mu + h_dn);          // U_mu(x-nu)
-        q.c2[i] = (nu == DEP_NU) ? ldq_dep(o_nu + h_dn) : ldq(o_nu + h_dn);  // U_nu(x-nu)
-        // su2_run's loop state is fetched behind the first six link loads: its round trip then
-        // overlaps theirs instead of preceding them (the n = 0 Philox call needs `sweep`)
-        if (i == 0) run_state(hp, sweep, inv_beta);
-    }
-#elif HB_ORDER == 3
     // First-touch loads first. CTAs sweep the lattice x fastest, then y, z, t; of the reads of one array in a
     // sub-step the one that reaches furthest ahead in that order misses L2, the others find the line the
     // earlier CTA brought in: U_nu(x+mu) is always ahead of U_nu(x-nu); U_nu(x+mu-nu) is ahead of U_nu(x)
@@ -151,41 +129,6 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
         q.b2[i] = DEP_MU ? ldq_dep(o_mu + h_dn) : ldq(o_mu + h_dn);                         // U_mu(x-nu)
         q.c2[i] = (nu == DEP_NU) ? ldq_dep(hp.oppo[nu] + h_dn) : ldq(hp.oppo[nu] + h_dn);  // U_nu(x-nu)
     }
-#else
-    // forward loads first: U_nu(x+mu) and U_nu(x+mu-nu) reach ahead of the CTA sweep through the lattice and are
-    // the ones that miss L2; issued as the first batch, the later batches only wait for cache hits
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        const int nu = i + (i >= MU ? 1 : 0);
-        q.a[i] = (nu == DEP_NU) ? ldq_dep(hp.oppo[nu] + h_up) : ldq(hp.oppo[nu] + h_up);  // U_nu(x+mu)
-    }
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        const int nu = i + (i >= MU ? 1 : 0);
-        q.a2[i] = ldq(hp.same[nu] + HB_CK((int)h_up + d.dn[nu]));  // U_nu(x+mu-nu)
-    }
-#if HB_ORDER == 2
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        const int nu = i + (i >= MU ? 1 : 0);
-        const uint32_t h_upnu = HB_CK(h + d.up[nu]);
-        q.b[i] = DEP_MU ? ldq_dep(o_mu + h_upnu) : ldq(o_mu + h_upnu);  // U_mu(x+nu)
-    }
-#endif
-    run_state(hp, sweep, inv_beta);
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        const int nu = i + (i >= MU ? 1 : 0);
-        const uint32_t h_dn = HB_CK(h + d.dn[nu]);
-#if HB_ORDER != 2
-        const uint32_t h_upnu = HB_CK(h + d.up[nu]);
-        q.b[i] = DEP_MU ? ldq_dep(o_mu + h_upnu) : ldq(o_mu + h_upnu);  // U_mu(x+nu)
-#endif
-        q.cc[i] = ldq(hp.same[nu] + HB_CK(h));                                            // U_nu(x)
-        q.b2[i] = DEP_MU ? ldq_dep(o_mu + h_dn) : ldq(o_mu + h_dn);                        // U_mu(x-nu)
-        q.c2[i] = (nu == DEP_NU) ? ldq_dep(hp.oppo[nu] + h_dn) : ldq(hp.oppo[nu] + h_dn);  // U_nu(x-nu)
-    }
-#endif
     return ix;
 }
 
@@ -325,7 +268,13 @@ struct MinBlocks<double> {
 
 // tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile;
 // grid = (nb0, nb1, nb2*nb3): x fastest, so CTAs are scheduled roughly in memory order.
-template <typename Real, int MU, int P, bool MEAS, bool ALT, int LHX, int LY, int LZ, int LT>
+// TLOOP: consecutive t-tiles one CTA walks through (kTLoop for the hot-path kernels of large fp32 lattices,
+// where a quarter of the CTA launches and drains is worth 4-5 %; 0 = g.tloop at run time, the ALT kernels).
+#ifndef HB_TLOOP
+#define HB_TLOOP 4
+#endif
+constexpr int kTLoop = HB_TLOOP;
+template <typename Real, int MU, int P, bool MEAS, bool ALT, int LHX, int LY, int LZ, int LT, int TLOOP>
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), (MinBlocks<Real>::value << 7) >> (LHX + LY + LZ + LT))
     heatbath_tiled_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
@@ -335,32 +284,19 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), (MinBlocks<Real>::v
         bzt -= rep * hp.nzt;
     }
     Site c = tile_site<LHX, LY, LZ, LT>(g, bzt);
+    // One CTA walks through `tloop` consecutive t-tiles: 65536 CTAs of 3.5 us each leave the
+    // SMs' CTA slots empty 6 % of the time between a drain and the next launch (ncu: 44 % warps active of 50 %).
+    const int tloop = TLOOP ? TLOOP : g.tloop;
+    const int tt = c.t & ((1 << LT) - 1);
+    c.t = (c.t - tt) * tloop + tt;
     if (ALT) c.t += g.t_lo;  // slab: the grid covers the interior slices only
-#ifdef HB_PF
-    // L2 prefetch (TMA unit) of the forward rows of the tile HB_PF z-t tile rows ahead in dispatch order:
-    // thread j < 6 * rows: array j / rows (three nu, both parities) at x+mu, row j % rows of that tile
-    if (!ALT) {
-        constexpr int ROWS = 1 << (LY + LZ + LT);
-        const int j = threadIdx.x;
-        const uint32_t bzt2 = bzt + HB_PF;
-        if (j < 6 * ROWS && bzt2 < (uint32_t)(g.nb[2] * g.nb[3])) {
-            const uint32_t bt2 = (g.nb[2] == 1) ? bzt2 : __umulhi(bzt2, g.zmagic);
-            const uint32_t bz2 = bzt2 - bt2 * (uint32_t)g.nb[2];
-            const int row = j & (ROWS - 1), a = j >> (LY + LZ + LT);  // a = 0..5
-            const int i = a >> 1, nu = i + (i >= MU ? 1 : 0);
-            int y = (int)(blockIdx.y << LY) + (row & ((1 << LY) - 1));
-            int z = (int)(bz2 << LZ) + ((row >> LY) & ((1 << LZ) - 1));
-            int t = (int)(bt2 << LT) + (row >> (LY + LZ));
-            if (MU == 1) y = (y + 1 == g.n[1]) ? 0 : y + 1;
-            if (MU == 2) z = (z + 1 == g.n[2]) ? 0 : z + 1;
-            if (MU == 3) t = (t + 1 == g.n[3]) ? 0 : t + 1;
-            const int h0 = (int)(blockIdx.x << LHX) + g.sy * y + g.sz * z + g.st * t;
-            const typename LinkPtr<Real>::type* src = ((a & 1) ? hp.same[nu] : hp.oppo[nu]) + h0;
-            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)(sizeof(*src) << LHX)) : "memory");
-        }
+    Real e = 0;
+    if (TLOOP == 1) {
+        e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err);
+    } else {
+#pragma unroll 1
+        for (int it = 0; it < tloop; ++it, c.t += 1 << LT) e += heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err);
     }
-#endif
-    const Real e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err);
     if (MEAS) {  // one fp64 partial per CTA, fixed order
         __shared__ double red[kBlock / 32];
         const double tot = block_sum_end((double)e, red);
@@ -422,9 +358,10 @@ __global__ void __launch_bounds__(kBlock)
     stq(links + (size_t)arr * g.vh + h, u);
 }
 
-void choose_tiling(Geom& g, int nrep)
+void choose_tiling(Geom& g, int nrep, int precision)
 {
     g.tile = -1;
+    g.tloop = 1;
     g.nb[0] = g.nb[1] = g.nb[2] = g.nb[3] = 0;
     g.zmagic = 0;
     for (int k = 0; k < kNumTiles; ++k) {
@@ -442,6 +379,9 @@ void choose_tiling(Geom& g, int nrep)
         g.nb[1] = (int)nb1;
         g.nb[2] = (int)nb2;
         g.nb[3] = (int)nb3;
+        // walk (see heatbath_tiled_kernel): fp32, first tile shape, and at least 4 CTA waves of 148 x 8 left
+        if (k == 0 && precision == 32 && nb3 % kTLoop == 0 && (uint64_t)g.nb[0] * nb1 * nb2 * (nb3 / kTLoop) >= 4736)
+            g.tloop = kTLoop;
         g.zmagic = (uint32_t)(((1ull << 32) + nb2 - 1) / nb2);  // unused if nb2 == 1
         return;
     }
@@ -480,15 +420,25 @@ static int launch_substep_t(void* links, const Geom& g, double beta, double creu
     hp.state = state;
     hp.reps = reps;
     hp.rep_stride = 8u * g.vh;
-    hp.nzt = (uint32_t)(g.nb[2] * g.nb[3]);
+    hp.nzt = (uint32_t)(g.nb[2] * (g.nb[3] / g.tloop));
     hp.epart_stride = (uint32_t)(3 * heatbath_ctas(g));
-    const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * g.nb[3] * nrep));
-    if (g.tile == 0) {
-        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3]>,
+    const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * (g.nb[3] / g.tloop) * nrep));
+    // hot-path kernels: the walk length is a template parameter (1, or kTLoop on the first tile shape in fp32);
+    // the ALT kernels read it from g
+    constexpr bool kWalk = !ALT && sizeof(Real) == 4;
+    if (g.tile == 0 && kWalk && g.tloop == kTLoop) {
+        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3],
+                                        kWalk ? kTLoop : 0>,
+                  grid, dim3(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3])), st, overlap, g, hp,
+                  err);
+    } else if (g.tile == 0) {
+        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3],
+                                        ALT ? 0 : 1>,
                   grid, dim3(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3])), st, overlap, g, hp,
                   err);
     } else if (g.tile == 1) {
-        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3]>,
+        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3],
+                                        ALT ? 0 : 1>,
                   grid, dim3(1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3])), st, overlap, g, hp,
                   err);
     } else {
@@ -501,7 +451,7 @@ static int launch_substep_t(void* links, const Geom& g, double beta, double creu
 // number of CTAs (= fused-plaquette partials) of one heat-bath launch
 size_t heatbath_ctas(const Geom& g)
 {
-    if (g.tile >= 0) return (size_t)g.nb[0] * g.nb[1] * g.nb[2] * g.nb[3];
+    if (g.tile >= 0) return (size_t)g.nb[0] * g.nb[1] * g.nb[2] * (g.nb[3] / g.tloop);
     return ((size_t)g.st * g.nt_upd + kBlock - 1) / kBlock;
 }
 

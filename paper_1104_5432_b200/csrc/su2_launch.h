@@ -65,7 +65,7 @@ struct SlabCtx {
 };
 
 // fills g.tile (index into kTiles or -1), g.nb and g.zmagic; nrep = replicas of a batch (grid z = replica x z-t tiles)
-void choose_tiling(Geom& g, int nrep = 1);
+void choose_tiling(Geom& g, int nrep = 1, int precision = 64);
 size_t partials_needed(const Geom& g);
 
 // each returns the number of kernels it enqueued (0 on launch failure; check cudaGetLastError)
