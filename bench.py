@@ -244,6 +244,19 @@ def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, 
     torch.cuda.synchronize()
     lat.synchronize()
     res["ms_per_step_run"] = s2.elapsed_time(e2) / steps
+    # ... and with the opt-in tail overlap (SU2_OPT_TAIL_OVERLAP): the Polyakov kernel of a step
+    # beside the next step's first six sub-steps
+    lat.set_option("tail_overlap", 1)
+    time.sleep(COOL_DOWN_S)
+    lat.run(beta, (1 << 21), 16, obs[:32] if obs.numel() >= 32 else torch.zeros(32, dtype=torch.float64, device=lat.device))
+    torch.cuda.synchronize()
+    s3, e3 = ev(), ev()
+    s3.record()
+    lat.run(beta, (1 << 21) + 16, steps, obs)
+    e3.record()
+    torch.cuda.synchronize()
+    lat.synchronize()
+    res["ms_per_step_run_tail_overlap"] = s3.elapsed_time(e3) / steps
     lat.close()
     del lat, obs
     torch.cuda.empty_cache()
@@ -655,7 +668,9 @@ def main():
         "init_ms": r["init_ms"], "plaquette_last": r["plaquette_last"], "polyakov_last": r["polyakov_last"],
         "su2_run": {"value": world * w.links / (r["ms_per_step_run"] * 1e-3), "unit": UNIT,
                     "ms_per_step": r["ms_per_step_run"],
-                    "what": "the same steps as one su2_run call (captured CUDA graph replayed), timed after the same cool-down"},
+                    "ms_per_step_tail_overlap": r["ms_per_step_run_tail_overlap"],
+                    "what": "the same steps as one su2_run call (captured CUDA graph replayed), timed after the same cool-down; "
+                            "tail_overlap = the same with SU2_OPT_TAIL_OVERLAP"},
     }
 
     if not args.headline_only and rank == 0:
@@ -672,6 +687,7 @@ def main():
                 "value": ww.links * args.steps / (rr["ms_total"] * 1e-3), "unit": UNIT,
                 "ms_per_step": rr["ms_per_step"], "ms_per_sweep": rr["sweep_ms"],
                 "plaquette_last": rr["plaquette_last"], "su2_run_ms_per_step": rr["ms_per_step_run"],
+                "su2_run_tail_overlap_ms_per_step": rr["ms_per_step_run_tail_overlap"],
             }
         line["workloads"] = others
         line["aux"] = time_aux(pkg, torch, workloads)

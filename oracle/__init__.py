@@ -132,40 +132,46 @@ def set_draw(method, mode="f64"):
     _check(getattr(lib(), f"orc_set_draw_{mode}")(DRAW[method]), "set_draw")
 
 
-def heatbath_link(dims, links, beta, seed, sweep, s, mu, mode="f64", return_k=False):
-    """New link of (site s, direction mu), lattice untouched. Returns (u, trials, margin[, k])."""
+def heatbath_link(dims, links, beta, seed, sweep, s, mu, mode="f64", return_k=False, return_delta=False):
+    """New link of (site s, direction mu), lattice untouched. Returns (u, trials, margin[, k][, delta])."""
     D, d = _dims(dims)
     u = np.zeros(4, dtype=_DT[mode])
     tr = C.c_int(0)
     mg = C.c_double(0)
-    kn = C.c_double(0)
+    kn, dl = C.c_double(0), C.c_double(0)
     rc = getattr(lib(), f"orc_heatbath_link_{mode}")(D, _p(d), _p(links), C.c_double(beta), C.c_uint64(seed),
                                                     C.c_uint32(sweep), C.c_int64(s), mu, _p(u), C.byref(tr),
-                                                    C.byref(mg), C.byref(kn))
+                                                    C.byref(mg), C.byref(kn), C.byref(dl))
     _check(rc, "heatbath_link")
-    return (u, tr.value, mg.value, kn.value) if return_k else (u, tr.value, mg.value)
+    out = (u, tr.value, mg.value)
+    if return_k:
+        out += (kn.value,)
+    if return_delta:
+        out += (dl.value,)
+    return out
 
 
 def heatbath_substep(dims, links, beta, seed, sweep, mu, parity, mode="f64", order=None, trials=None, margin=None,
-                     knorm=None):
-    """In place on `links`. trials: int32 [V][D]; margin, knorm (staple norm k of each updated link):
-    float64 [V][D]; all optional, only the entries of the updated links are written."""
+                     knorm=None, delta=None):
+    """In place on `links`. trials: int32 [V][D]; margin, knorm (staple norm k of each updated link), delta
+    (the accepted 1 - x0 of its draw): float64 [V][D]; all optional, only the entries of the updated links
+    are written."""
     D, d = _dims(dims)
     assert links.dtype == _DT[mode] and links.flags.c_contiguous
     if order is not None:
         order = np.ascontiguousarray(order, dtype=np.int64)
     rc = getattr(lib(), f"orc_heatbath_substep_{mode}")(D, _p(d), _p(links), C.c_double(beta), C.c_uint64(seed),
                                                        C.c_uint32(sweep), mu, parity, _p(order), _p(trials),
-                                                       _p(margin), _p(knorm))
+                                                       _p(margin), _p(knorm), _p(delta))
     _check(rc, "heatbath_substep")
 
 
-def heatbath_sweep(dims, links, beta, seed, sweep, mode="f64", trials=None, margin=None, knorm=None):
-    """In place on `links`. trials: int32 [V][D]; margin, knorm: float64 [V][D] (all optional)."""
+def heatbath_sweep(dims, links, beta, seed, sweep, mode="f64", trials=None, margin=None, knorm=None, delta=None):
+    """In place on `links`. trials: int32 [V][D]; margin, knorm, delta: float64 [V][D] (all optional)."""
     D, d = _dims(dims)
     assert links.dtype == _DT[mode] and links.flags.c_contiguous
     rc = getattr(lib(), f"orc_heatbath_sweep_{mode}")(D, _p(d), _p(links), C.c_double(beta), C.c_uint64(seed),
-                                                     C.c_uint32(sweep), _p(trials), _p(margin), _p(knorm))
+                                                     C.c_uint32(sweep), _p(trials), _p(margin), _p(knorm), _p(delta))
     _check(rc, "heatbath_sweep")
 
 

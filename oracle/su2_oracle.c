@@ -460,10 +460,12 @@ int FN(orc_creutz_x0)(double alpha, uint64_t seed, uint32_t s, uint32_t sweep, d
 /* *knorm (nullable) = the staple norm k of this link as the update saw it: the draw divides the
  * staple by it (Vbar = v/k), so 1/k is the factor by which a perturbation of the neighbouring
  * links reaches the new link - the parity harness classifies ill-conditioned links with it
- * (DESIGN.md 3 [R13b]). */
+ * (DESIGN.md 3 [R13b]). *delta (nullable) = the accepted delta = 1 - x0 of the draw: the vector part of X
+ * lives on a sphere of radius sqrt(delta (2 - delta)), which amplifies a rounding of delta by
+ * |1 - delta| / radius (same use). */
 static int heatbath_link(const geom_t *g, const REAL *links, double beta, uint64_t seed,
                          uint32_t sweep, int64_t s, int mu, AREAL unew[4], int *trials, AREAL *margin,
-                         double *knorm)
+                         double *knorm, double *delta_out)
 {
     int x[ORC_MAXD];
     site_coords(g, s, x);
@@ -480,6 +482,7 @@ static int heatbath_link(const geom_t *g, const REAL *links, double beta, uint64
         if (trials) *trials = 0;
         if (margin) *margin = (AREAL)1;
         if (knorm) *knorm = 0.0;
+        if (delta_out) *delta_out = 1.0;
         return ORC_OK;
     }
     AREAL k = A_SQRT(k2);
@@ -498,6 +501,8 @@ static int heatbath_link(const geom_t *g, const REAL *links, double beta, uint64
         if (mc < 0) mc = -mc;
         if (mc < *margin) *margin = mc;
     }
+
+    if (delta_out) *delta_out = (double)delta;
 
     /* [R7] direction uniform on the sphere of radius sqrt(1-x0^2) = sqrt(delta(2-delta)) */
     AREAL x0 = (AREAL)1 - delta;
@@ -525,12 +530,12 @@ static int heatbath_link(const geom_t *g, const REAL *links, double beta, uint64
 /* one link, result returned, lattice untouched (single-link pins) */
 int FN(orc_heatbath_link)(int D, const int *dims, const REAL *links, double beta, uint64_t seed,
                           uint32_t sweep, int64_t s, int mu, REAL *u_out, int *trials, double *margin,
-                          double *knorm)
+                          double *knorm, double *delta)
 {
     geom_t g;
     if (geom_init(&g, D, dims) || s < 0 || s >= g.V || mu < 0 || mu >= D || !(beta > 0)) return ORC_EARG;
     AREAL u[4], m;
-    int rc = heatbath_link(&g, links, beta, seed, sweep, s, mu, u, trials, &m, knorm);
+    int rc = heatbath_link(&g, links, beta, seed, sweep, s, mu, u, trials, &m, knorm, delta);
     if (rc) return rc;
     for (int c = 0; c < 4; ++c) u_out[c] = (REAL)u[c];
     if (margin) *margin = (double)m;
@@ -540,10 +545,10 @@ int FN(orc_heatbath_link)(int D, const int *dims, const REAL *links, double beta
 /* One sub-step (mu, parity) [R4]: every U_mu(x) with parity(x) = parity, in
  * place. `order` (nullable) is a permutation of 0..V-1 giving the visiting
  * order of the sites (order-independence pin); NULL = ascending s.
- * trials/margin/knorm (nullable) are indexed [s*D+mu]. */
+ * trials/margin/knorm/delta (nullable) are indexed [s*D+mu]. */
 int FN(orc_heatbath_substep)(int D, const int *dims, REAL *links, double beta, uint64_t seed,
                              uint32_t sweep, int mu, int parity, const int64_t *order,
-                             int32_t *trials, double *margin, double *knorm)
+                             int32_t *trials, double *margin, double *knorm, double *delta)
 {
     geom_t g;
     if (geom_init(&g, D, dims) || mu < 0 || mu >= D || (parity != 0 && parity != 1) || !(beta > 0) ||
@@ -556,26 +561,27 @@ int FN(orc_heatbath_substep)(int D, const int *dims, REAL *links, double beta, u
         if (site_parity(&g, x) != parity) continue;
         AREAL u[4], m;
         int tr;
-        double kn;
-        int rc = heatbath_link(&g, links, beta, seed, sweep, s, mu, u, &tr, &m, &kn);
+        double kn, dl;
+        int rc = heatbath_link(&g, links, beta, seed, sweep, s, mu, u, &tr, &m, &kn, &dl);
         if (rc) return rc;
         REAL *dst = links + (s * D + mu) * 4;
         for (int c = 0; c < 4; ++c) dst[c] = (REAL)u[c];
         if (trials) trials[s * D + mu] = tr;
         if (margin) margin[s * D + mu] = (double)m;
         if (knorm) knorm[s * D + mu] = kn;
+        if (delta) delta[s * D + mu] = dl;
     }
     return ORC_OK;
 }
 
 /* One sweep [R4]: for mu = 0..D-1: for parity = 0, 1: sub-step(mu, parity). */
 int FN(orc_heatbath_sweep)(int D, const int *dims, REAL *links, double beta, uint64_t seed,
-                           uint32_t sweep, int32_t *trials, double *margin, double *knorm)
+                           uint32_t sweep, int32_t *trials, double *margin, double *knorm, double *delta)
 {
     for (int mu = 0; mu < D; ++mu)
         for (int parity = 0; parity < 2; ++parity) {
             int rc = FN(orc_heatbath_substep)(D, dims, links, beta, seed, sweep, mu, parity, NULL, trials, margin,
-                                              knorm);
+                                              knorm, delta);
             if (rc) return rc;
         }
     return ORC_OK;

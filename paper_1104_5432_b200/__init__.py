@@ -21,7 +21,7 @@ SU2_OK, SU2_EARG, SU2_EALLOC, SU2_ECUDA, SU2_ESTATE = 0, 1, 2, 3, 4
 SU2_START_COLD, SU2_START_HOT = 0, 1
 SU2_DRAW_KP, SU2_DRAW_AUTO, SU2_DRAW_CREUTZ = 0, 1, 2
 SU2_ALPHA_C = 1.6847
-SU2_OPT_OVERLAP, SU2_OPT_RUN_GRAPH = 0, 1
+SU2_OPT_OVERLAP, SU2_OPT_RUN_GRAPH, SU2_OPT_TAIL_OVERLAP = 0, 1, 2
 SU2_PROBE_READ, SU2_PROBE_COPY = 0, 1
 
 _lib = None
@@ -373,7 +373,7 @@ class Lattice:
         su2_set_draw(self.h, {"kp": SU2_DRAW_KP, "auto": SU2_DRAW_AUTO, "creutz": SU2_DRAW_CREUTZ}[method])
 
     def set_option(self, option, value):
-        su2_set_option(self.h, {"overlap": SU2_OPT_OVERLAP, "run_graph": SU2_OPT_RUN_GRAPH}[option], value)
+        su2_set_option(self.h, {"overlap": SU2_OPT_OVERLAP, "run_graph": SU2_OPT_RUN_GRAPH, "tail_overlap": SU2_OPT_TAIL_OVERLAP}[option], value)
 
     def sweep(self, beta, sweep_idx):
         su2_heatbath_sweep(self.h, beta, sweep_idx)

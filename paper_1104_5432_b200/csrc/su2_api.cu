@@ -30,6 +30,10 @@ struct su2_lattice {
     cudaEvent_t run_ev_in, run_ev_out;
     cudaGraphExec_t run_exec;
     bool run_graphs;   // su2_run replays a captured CUDA graph (su2_set_option SU2_OPT_RUN_GRAPH)
+    bool tail_overlap; // su2_run: the Polyakov kernel of a step runs beside the next step (SU2_OPT_TAIL_OVERLAP)
+    cudaStream_t tail_stream;
+    cudaEvent_t ev_fork, ev_join;
+    int run_block;     // steps per captured graph (1, or kRunBlock with tail overlap)
     double creutz_below;  // [R15] su2_set_draw: 0 (KP), SU2_ALPHA_C (auto) or +inf (Creutz)
     // replica batch: nrep configurations one after the other from links_base; `links`,
     // `seed` and `initialised` are those of the selected replica (single-lattice calls act on it)
@@ -170,11 +174,11 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, int nrep, 
     lat->sc.n_partials = partials_needed(g);
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.partials, lat->sc.n_partials * sizeof(double));
     lat->links_base = lat->links;
-    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.epart, (size_t)nrep * 3 * heatbath_ctas(g) * sizeof(double));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.epart, 2 * (size_t)nrep * 3 * heatbath_ctas(g) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.field, (size_t)nrep * v3 * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.reps, (size_t)nrep * sizeof(RepParams));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.out, (2 + kMaxR) * sizeof(double));
-    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.state, kRunCopies * sizeof(RunState));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.state, 2 * kRunCopies * sizeof(RunState));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.slots, (size_t)nrep * 2 * (v3 / 64 + 1) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.ticket, (size_t)nrep * sizeof(unsigned));
     if (ce == cudaSuccess) ce = cudaMemset(lat->sc.ticket, 0, (size_t)nrep * sizeof(unsigned));
@@ -235,6 +239,9 @@ extern "C" int su2_lattice_destroy(su2_lattice* lat)
     if (lat->run_ev_in) cudaEventDestroy(lat->run_ev_in);
     if (lat->run_ev_out) cudaEventDestroy(lat->run_ev_out);
     if (lat->run_stream) cudaStreamDestroy(lat->run_stream);
+    if (lat->ev_fork) cudaEventDestroy(lat->ev_fork);
+    if (lat->ev_join) cudaEventDestroy(lat->ev_join);
+    if (lat->tail_stream) cudaStreamDestroy(lat->tail_stream);
     delete lat;
     return SU2_OK;
 }
@@ -266,6 +273,7 @@ extern "C" int su2_set_option(su2_lattice* lat, int option, int value)
     switch (option) {
         case SU2_OPT_OVERLAP: lat->pdl = value != 0; break;
         case SU2_OPT_RUN_GRAPH: lat->run_graphs = value != 0; break;
+        case SU2_OPT_TAIL_OVERLAP: lat->tail_overlap = value != 0; break;
         default: return fail(lat, SU2_EARG, "su2_set_option: unknown option");
     }
     drop_run_graph(lat);  // the captured step was built with the other setting
@@ -444,31 +452,64 @@ extern "C" int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_
     return SU2_OK;
 }
 
-// one step of su2_run on stream `st`, every per-step quantity read from the device RunState
-static void enqueue_run_step(su2_lattice* lat, cudaStream_t st, bool allow_overlap)
+// Steps of su2_run on stream `st`, every per-step quantity read from a device RunState.
+// Plain mode (tail_st == NULL): 8 sub-steps + the Polyakov kernel with the step tail, all on `st`, one loop state.
+// Tail overlap: the Polyakov kernel reads only U_t, which the next step does not write before its
+// sub-step (3,0), so it runs on `tail_st` beside the next step's first six sub-steps: forked behind (3,1), joined
+// before the next (3,0). What the two then touch at the same time alternates between two sets by step parity:
+// the fused-plaquette partials (written by (1,1), (2,1), (3,1), read by the tail) and the loop state (read by the
+// sub-steps, advanced - by 2 - by the tail). Same kernels on the same inputs: bit-identical results.
+static const int kRunBlock = 8;  // steps per captured graph with tail overlap (graph launches serialise: the last
+                                 // tail of a block is not overlapped)
+static void enqueue_run_steps(su2_lattice* lat, cudaStream_t st, cudaStream_t tail_st, int count, bool allow_overlap)
 {
     const size_t ctas = heatbath_ctas(lat->g);
-    lat->last_substep = -1;
-    for (int mu = 0; mu < 4; ++mu)
-        for (int p = 0; p < 2; ++p)
-            enqueue_substep(lat, 1.0, 0u, mu, p, (p == 1 && mu >= 1) ? lat->sc.epart + (mu - 1) * ctas : nullptr,
-                            lat->sc.state, st, allow_overlap);
-    lat->launches += launch_polyakov_step(lat->links, lat->g, lat->precision, lat->sc, lat->sc.epart, 3 * ctas,
-                                          1.0 / (6.0 * 2.0 * (double)lat->g.vh), nullptr, lat->sc.state,
-                                          allow_overlap && lat->pdl, st);
+    const double scale = 1.0 / (6.0 * 2.0 * (double)lat->g.vh);
+    bool pending_join = false;
+    for (int i = 0; i < count; ++i) {
+        const int e = tail_st ? (i & 1) : 0;
+        double* epart = lat->sc.epart + (size_t)e * 3 * ctas;
+        RunState* state = lat->sc.state + (size_t)e * kRunCopies;
+        lat->last_substep = -1;
+        for (int mu = 0; mu < 4; ++mu)
+            for (int p = 0; p < 2; ++p) {
+                bool ov = allow_overlap;
+                if (tail_st && mu == 3 && p == 0 && pending_join) {  // the previous tail still reads U_t
+                    cudaStreamWaitEvent(st, lat->ev_join, 0);
+                    pending_join = false;
+                    ov = false;  // two predecessors: launched fully serialised
+                }
+                enqueue_substep(lat, 1.0, 0u, mu, p, (p == 1 && mu >= 1) ? epart + (mu - 1) * ctas : nullptr, state, st, ov);
+            }
+        if (tail_st) {
+            cudaEventRecord(lat->ev_fork, st);
+            cudaStreamWaitEvent(tail_st, lat->ev_fork, 0);
+            lat->launches += launch_polyakov_step(lat->links, lat->g, lat->precision, lat->sc, epart, 3 * ctas, scale,
+                                                  nullptr, state, false, tail_st, 1, 2u);
+            cudaEventRecord(lat->ev_join, tail_st);
+            pending_join = true;
+            lat->last_substep = 7;  // the next (0,0) follows (3,1) on `st`
+        } else {
+            lat->launches += launch_polyakov_step(lat->links, lat->g, lat->precision, lat->sc, epart, 3 * ctas, scale,
+                                                  nullptr, state, allow_overlap && lat->pdl, st);
+            lat->last_substep = kAfterStepTail;
+        }
+    }
+    if (pending_join) cudaStreamWaitEvent(st, lat->ev_join, 0);
     lat->last_substep = -1;
 }
 
-// capture one step into an executable graph; with programmatic edges first, without if the
+// capture `count` steps into an executable graph; with programmatic edges first, without if the
 // driver refuses them
-static bool build_run_graph(su2_lattice* lat)
+static bool build_run_graph(su2_lattice* lat, int count)
 {
+    cudaStream_t tail = lat->tail_overlap ? lat->tail_stream : nullptr;
     for (int attempt = 0; attempt < 2 && !lat->run_exec; ++attempt) {
         const bool overlap = attempt == 0;
         const uint64_t launches0 = lat->launches;
         cudaGraph_t graph = nullptr;
         if (cudaStreamBeginCapture(lat->run_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
-        enqueue_run_step(lat, lat->run_stream, overlap);
+        enqueue_run_steps(lat, lat->run_stream, tail, count, overlap);
         cudaError_t ce = cudaStreamEndCapture(lat->run_stream, &graph);
         lat->launches = launches0;  // captured, not launched
         if (ce == cudaSuccess && graph) ce = cudaGraphInstantiate(&lat->run_exec, graph, 0);
@@ -478,6 +519,7 @@ static bool build_run_graph(su2_lattice* lat)
             cudaGetLastError();
         }
     }
+    lat->run_block = count;
     return lat->run_exec != nullptr;
 }
 
@@ -494,20 +536,32 @@ extern "C" int su2_run(su2_lattice* lat, double beta, uint32_t sweep_idx0, uint3
         CK(lat, cudaEventCreateWithFlags(&lat->run_ev_in, cudaEventDisableTiming));
         CK(lat, cudaEventCreateWithFlags(&lat->run_ev_out, cudaEventDisableTiming));
     }
+    if (lat->tail_overlap && !lat->tail_stream) {
+        CK(lat, cudaStreamCreateWithFlags(&lat->tail_stream, cudaStreamNonBlocking));
+        CK(lat, cudaEventCreateWithFlags(&lat->ev_fork, cudaEventDisableTiming));
+        CK(lat, cudaEventCreateWithFlags(&lat->ev_join, cudaEventDisableTiming));
+    }
+    cudaStream_t tail = lat->tail_overlap ? lat->tail_stream : nullptr;
     // the private stream continues the handle's stream and hands back to it
     CK(lat, cudaEventRecord(lat->run_ev_in, lat->stream));
     CK(lat, cudaStreamWaitEvent(lat->run_stream, lat->run_ev_in, 0));
+    // loop state: one set, or two alternating by step parity (set e starts at step e and advances by 2)
     lat->launches += launch_set_run_state(lat->sc.state, 1.0 / beta, dev_out, sweep_idx0, 0u, lat->run_stream);
-    const bool graphs = lat->run_graphs && (lat->run_exec || build_run_graph(lat));
+    if (tail)
+        lat->launches += launch_set_run_state(lat->sc.state + kRunCopies, 1.0 / beta, dev_out, sweep_idx0 + 1u, 1u,
+                                              lat->run_stream);
+    const int block = tail ? kRunBlock : 1;
+    const bool graphs = lat->run_graphs && (lat->run_exec || build_run_graph(lat, block));
     const uint64_t per_step = 8 + 1;
-    for (uint32_t i = 0; i < n_steps; ++i) {
-        if (graphs) {
+    uint32_t done = 0;
+    if (graphs)
+        for (; done + (uint32_t)block <= n_steps; done += (uint32_t)block) {
             CK(lat, cudaGraphLaunch(lat->run_exec, lat->run_stream));
-            lat->launches += per_step;
-        } else {
-            enqueue_run_step(lat, lat->run_stream, true);
+            lat->launches += per_step * (uint64_t)block;
         }
-    }
+    // the remainder of a block (or everything, without graphs) is enqueued directly; a block is an even number of
+    // steps, so the parity of the remaining steps starts at 0 again
+    if (done < n_steps) enqueue_run_steps(lat, lat->run_stream, tail, (int)(n_steps - done), true);
     CK(lat, cudaGetLastError());
     CK(lat, cudaEventRecord(lat->run_ev_out, lat->run_stream));
     CK(lat, cudaStreamWaitEvent(lat->stream, lat->run_ev_out, 0));

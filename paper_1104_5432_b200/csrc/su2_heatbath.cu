@@ -273,6 +273,9 @@ struct MinBlocks<double> {
 #ifndef HB_TLOOP
 #define HB_TLOOP 4
 #endif
+#ifndef HB_WALK_F64
+#define HB_WALK_F64 0
+#endif
 constexpr int kTLoop = HB_TLOOP;
 template <typename Real, int MU, int P, bool MEAS, bool ALT, int LHX, int LY, int LZ, int LT, int TLOOP>
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), (MinBlocks<Real>::value << 7) >> (LHX + LY + LZ + LT))
@@ -380,7 +383,7 @@ void choose_tiling(Geom& g, int nrep, int precision)
         g.nb[2] = (int)nb2;
         g.nb[3] = (int)nb3;
         // walk (see heatbath_tiled_kernel): fp32, first tile shape, and at least 4 CTA waves of 148 x 8 left
-        if (k == 0 && precision == 32 && nb3 % kTLoop == 0 && (uint64_t)g.nb[0] * nb1 * nb2 * (nb3 / kTLoop) >= 4736)
+        if (k == 0 && (precision == 32 || HB_WALK_F64) && nb3 % kTLoop == 0 && (uint64_t)g.nb[0] * nb1 * nb2 * (nb3 / kTLoop) >= 4736)
             g.tloop = kTLoop;
         g.zmagic = (uint32_t)(((1ull << 32) + nb2 - 1) / nb2);  // unused if nb2 == 1
         return;
@@ -425,7 +428,10 @@ static int launch_substep_t(void* links, const Geom& g, double beta, double creu
     const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * (g.nb[3] / g.tloop) * nrep));
     // hot-path kernels: the walk length is a template parameter (1, or kTLoop on the first tile shape in fp32);
     // the ALT kernels read it from g
-    constexpr bool kWalk = !ALT && sizeof(Real) == 4;
+#ifndef HB_WALK_F64
+#define HB_WALK_F64 0
+#endif
+    constexpr bool kWalk = !ALT && (sizeof(Real) == 4 || HB_WALK_F64);
     if (g.tile == 0 && kWalk && g.tloop == kTLoop) {
         launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3],
                                         kWalk ? kTLoop : 0>,

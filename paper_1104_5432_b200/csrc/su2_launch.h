@@ -44,11 +44,12 @@ inline void launch_ex(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStrea
 struct Scratch {
     double* partials;   // [device] block partial sums (plaquette | polyakov | correlator)
     size_t n_partials;  // capacity in doubles
-    double* epart;      // [device] fused plaquette partials: 3 * heatbath_ctas(g) doubles
+    double* epart;      // [device] fused plaquette partials: 2 sets (su2_run's tail overlap alternates them) of
+                        // 3 * heatbath_ctas(g) doubles per replica
     double* field;      // [device] l(x) of the Polyakov kernel, V/Nt doubles
     double* out;        // [device] 2 + kMaxR doubles: plaquette, polyakov, correlator
     int* err;           // [device] sticky error flags (bit 0: KP trial cap hit)
-    RunState* state;    // [device] loop state of su2_run
+    RunState* state;    // [device] loop state of su2_run: 2 sets of kRunCopies copies
     double* slots;      // [device] step tail: 2 doubles per CTA of the Polyakov kernel (<= V/Nt/64 + 1 CTAs), per replica
     unsigned* ticket;   // [device] step tail: arrival counters (one per replica), zero between steps
     RepParams* reps;    // [device] batch: per-replica 1/beta and seed
@@ -84,7 +85,7 @@ int launch_polyakov_partials(const void* links, const Geom& g, int precision, co
                              cudaStream_t st);
 int launch_polyakov_step(const void* links, const Geom& g, int precision, const Scratch& sc, const double* epart,
                          size_t n_epart, double scale_plaq, double* dev_dst, RunState* state, bool overlap,
-                         cudaStream_t st, int nrep = 1);
+                         cudaStream_t st, int nrep = 1, unsigned advance = 1);
 // `scale` = 0: 1 / (number of plaquettes of g); a slab passes 1 / (plaquettes of the whole lattice)
 int launch_plaquette(const void* links, const Geom& g, int precision, const Scratch& sc, double* dev_dst,
                      cudaStream_t st, double scale = 0.0);

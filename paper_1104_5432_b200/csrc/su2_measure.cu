@@ -143,6 +143,7 @@ struct StepTail {
     unsigned* ticket;     // [device] one per replica, zero between steps
     double* dst;          // [device] 2 doubles per replica (ignored when state != NULL)
     RunState* state;      // su2_run: destination state->out[2*index..], then sweep and index advance
+    unsigned advance;     // ... by this much (1; 2 when two loop states alternate)
 };
 __device__ __forceinline__ void step_tail(const StepTail& tl, double poly_tot, double* red)
 {
@@ -180,8 +181,8 @@ __device__ __forceinline__ void step_tail(const StepTail& tl, double poly_tot, d
     }
     if (tl.state)  // su2_run: advance every copy of the loop state (this CTA is the last one running)
         for (int i = threadIdx.x; i < kRunCopies; i += blockDim.x) {
-            tl.state[i].sweep += 1u;
-            tl.state[i].index += 1u;
+            tl.state[i].sweep += tl.advance;
+            tl.state[i].index += tl.advance;
         }
 }
 
@@ -504,10 +505,10 @@ int launch_polyakov_partials(const void* links, const Geom& g, int precision, co
 // the last kernel of a step: Polyakov loop + both final sums (see step_tail)
 int launch_polyakov_step(const void* links, const Geom& g, int precision, const Scratch& sc, const double* epart,
                          size_t n_epart, double scale_plaq, double* dev_dst, RunState* state, bool overlap,
-                         cudaStream_t st, int nrep)
+                         cudaStream_t st, int nrep, unsigned advance)
 {
     const uint64_t v3 = (uint64_t)g.n[0] * g.n[1] * g.n[2];
-    const StepTail tl = {epart, n_epart, scale_plaq, 1.0 / (double)v3, sc.slots, sc.ticket, dev_dst, state};
+    const StepTail tl = {epart, n_epart, scale_plaq, 1.0 / (double)v3, sc.slots, sc.ticket, dev_dst, state, advance};
     if (precision == 32)
         launch_polyakov_t<float>(links, g, sc, tl, overlap, st, nrep);
     else

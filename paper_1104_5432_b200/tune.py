@@ -4,7 +4,7 @@ knobs of csrc/, set through SU2HB_NVCC_EXTRA, e.g.
 
     SU2HB_NVCC_EXTRA="-DHB_T0=3 -DHB_T1=2 -DHB_T2=1 -DHB_T3=1" python -m paper_1104_5432_b200.build --force
     python -m paper_1104_5432_b200.tune            # one JSON line: ms per sweep, fraction of the HBM copy peak
-    python -m paper_1104_5432_b200.tune --one      # two sweeps per point and nothing else (for ncu)
+    python -m paper_1104_5432_b200.tune --one      # two sweeps + one su2_measure per point, no timing (for ncu)
 
 Burst = 40 (64^4) / 300 (32^4) sweeps after 2 s of idle; sustained = the second half of a further 1.2 s of
 continuous sweeps. A `links` signature (sha256 of small lattices after three sweeps) shows at a glance that a
@@ -37,7 +37,7 @@ def main():
             lat.init("hot", 1)
             lat.sweep(args.beta, 0)
             lat.sweep(args.beta, 1)
-            lat.synchronize()
+            lat.measure()  # the standalone plaquette and Polyakov kernels
             lat.close()
         return 0
     peak = 6539.9

@@ -13,10 +13,17 @@ Tolerances are BASELINE.json north_star's: every link after one sweep |d| <= 1e-
                      and the deviations the 18 input links already carry when earlier sub-steps of the
                      same sweep wrote them, |dv| <= 2 S_in, S_in = the sum of their measured |d| (the 2
                      turns the max-norm of d into a bound on the quaternion norm). The link's tolerance is
-                         max(TOL, (E_V + 2 S_in) / k),   k = the oracle's staple norm for that link:
-                     north_star's 1e-5 wherever the update is well conditioned (k >= 0.2, clean inputs),
-                     wider only by what 1/k explains. Links that need the wider bound are counted against
-                     conditioned_budget().
+                         max(TOL, (E_V + 2 S_in) / k),   k = the oracle's staple norm for that link.
+                     A second amplifier sits in the draw itself: the vector part of X lives on a sphere of
+                     radius rad = sqrt(delta (2 - delta)) [R7], so a rounding of delta = 1 - x0 (two fp32
+                     evaluations of -(ln R + cos^2 ln R'')/alpha differ by <= E_D (delta + 1/alpha), E_D = 4e-7:
+                     a few ulp of the sum, or the MUFU budget of DESIGN.md 6.2) moves it by that times
+                     |1 - delta| / rad - unbounded as x0 -> +-1, probability ~1e-6 per link. With the oracle's
+                     delta for the link:
+                         tol = max(TOL, (E_V + 2 S_in) / k + E_D (delta + 1/alpha) max(1, |1 - delta| / rad)),
+                     north_star's 1e-5 wherever the update is well conditioned (k >= 0.2, clean inputs,
+                     rad >~ 0.05), wider only by what the two amplifiers explain. Links that need the wider
+                     bound are counted against conditioned_budget().
   downstream         a link whose staple contains a flipped link (or a link downstream of one) that was
                      updated earlier in the same sweep: not comparable and not counted; every OTHER link
                      is checked. (Its inputs deviate by O(1), so it also satisfies the bound above.)
@@ -39,6 +46,7 @@ PTOL = {64: 1e-12, 32: 1e-6}
 FLIP_MARGIN = {64: 1e-11, 32: 1e-5}
 MODE = {64: "f64", 32: "f32"}
 E_V = {64: 0.0, 32: 2e-6}  # rounding bound of the fp32 staple sum; fp64 has no conditioning excuse
+E_D = {64: 0.0, 32: 4e-7}  # rounding bound of the fp32 delta, in units of (delta + 1/alpha)
 # measured on B200 (profiles/r02a.md): 0 flips in 1.26e7 teacher-forced fp32 link updates at 32^4 (beta 2.3
 # and 6.0), 20 of which had an accept margin < 1e-6, i.e. ~1.6e-7 flips per link expected at the ~1e-7
 # rounding of the accept test. FLIP_RATE is the 95 % upper limit 3 / 1.26e7.
@@ -98,6 +106,25 @@ def staple_inputs_sum(T, mu):
     return _staple_inputs(T, mu, np.add)
 
 
+class Records:
+    """What the oracle records per updated link for the protocol: smallest accept margin, staple norm k,
+    accepted delta = 1 - x0. Pass **rec.kw to oracle.heatbath_substep / heatbath_sweep."""
+
+    def __init__(self, V):
+        self.margin, self.knorm, self.delta = np.ones((V, 4)), np.ones((V, 4)), np.ones((V, 4))
+
+    @property
+    def kw(self):
+        return dict(margin=self.margin, knorm=self.knorm, delta=self.delta)
+
+
+def draw_term(delta, k, beta, prec):
+    """E_D (delta + 1/alpha) max(1, |1 - delta| / rad): what a rounding of delta does to the new link"""
+    alpha = np.maximum(beta * k, 1e-30)
+    rad = np.sqrt(np.maximum(delta * (2.0 - delta), 1e-30))
+    return E_D[prec] * (delta + 1.0 / alpha) * np.maximum(1.0, np.abs(1.0 - delta) / rad)
+
+
 class Report:
     def __init__(self, flips, conditioned, downstream, worst):
         self.flips, self.conditioned, self.downstream, self.worst = flips, conditioned, downstream, worst
@@ -110,21 +137,22 @@ class Report:
         return f"Report(flips={self.flips}, conditioned={self.conditioned}, downstream={self.downstream}, worst={self.worst:.3e})"
 
 
-def compare_links(gpu, ora, dims, prec, substeps, margin=None, knorm=None, max_flips=None, max_conditioned=None,
+def compare_links(gpu, ora, dims, prec, substeps, rec=None, beta=None, max_flips=None, max_conditioned=None,
                   haar=True, what=""):
     """gpu, ora: [V][4][4] after the sub-steps `substeps` (list of (mu, parity) in execution order, every link
-    updated at most once) run on both sides from a common configuration; margin, knorm: the oracle's [V][4]
-    records of those sub-steps. Asserts the protocol above; returns a Report."""
+    updated at most once) run on both sides at coupling `beta` from a common configuration; rec: the oracle's
+    Records of those sub-steps. Asserts the protocol above; returns a Report."""
     nx, ny, nz, nt = dims
     shape = (nt, nz, ny, nx, 4)
     d = np.abs(gpu.astype(np.float64) - ora.astype(np.float64)).max(-1).reshape(shape)
     bad = d > TOL[prec]
     if not bad.any():
         return Report(0, 0, 0, float(d.max()))
-    assert margin is not None and knorm is not None, f"{what}: {int(bad.sum())} links differ, max {d.max():.3e}"
+    assert rec is not None and beta is not None, f"{what}: {int(bad.sum())} links differ, max {d.max():.3e}"
     assert len(set(substeps)) == len(substeps)
-    mg = np.asarray(margin).reshape(shape)
-    kn = np.asarray(knorm).reshape(shape)
+    mg = np.asarray(rec.margin).reshape(shape)
+    kn = np.asarray(rec.knorm).reshape(shape)
+    dl = np.asarray(rec.delta).reshape(shape)
     par = parity_grid(dims)
     taint = np.zeros(shape, bool)  # flipped links and what is downstream of them
     dev = np.zeros(shape)          # measured deviation of the links updated so far
@@ -136,13 +164,16 @@ def compare_links(gpu, ora, dims, prec, substeps, margin=None, knorm=None, max_f
         down = staple_inputs_any(taint, mu) & sel
         flip = b & ~down & (m < FLIP_MARGIN[prec])
         s_in = staple_inputs_sum(dev, mu)
-        cond = b & ~down & ~flip & (k > 0) & (dd * k <= E_V[prec] + 2.0 * s_in) & (E_V[prec] > 0)
+        kk = np.maximum(k, 1e-30)
+        allowed = (E_V[prec] + 2.0 * s_in) / kk + draw_term(dl[..., mu], kk, beta, prec)
+        cond = b & ~down & ~flip & (k > 0) & (dd <= allowed) & (E_V[prec] > 0)
         unexplained = b & ~down & ~flip & ~cond
         if unexplained.any():
             i = np.unravel_index(np.argmax(np.where(unexplained, dd, 0)), dd.shape)
             raise AssertionError(f"{what} sub-step mu={mu} p={p}: {int(unexplained.sum())} links differ beyond "
                                  f"tolerance with no excuse; worst |d|={dd[i]:.3e} at (t,z,y,x)={i}, accept margin "
-                                 f"{m[i]:.3e}, staple norm k={k[i]:.3e}, deviation of its inputs {s_in[i]:.3e}")
+                                 f"{m[i]:.3e}, staple norm k={k[i]:.3e}, deviation of its inputs {s_in[i]:.3e}, "
+                                 f"delta={dl[..., mu][i]:.6e}, allowed {allowed[i]:.3e}")
         n_flip += int(flip.sum())
         n_cond += int(cond.sum())
         n_down += int((b & down).sum())
@@ -158,13 +189,13 @@ def compare_links(gpu, ora, dims, prec, substeps, margin=None, knorm=None, max_f
     return Report(n_flip, n_cond, n_down, float(d.max()))
 
 
-def sampled_link_excused(d, margin, k, prec):
+def sampled_link_excused(d, margin, k, delta, beta, prec):
     """One sampled link outside tolerance (full-size tests recompute single links with
     oracle.heatbath_link from the pre-update configuration, so the inputs are clean and nothing is
     downstream): 'flip' [R13], 'conditioned' [R13b] or None."""
     if margin < FLIP_MARGIN[prec]:
         return "flip"
-    if k > 0 and E_V[prec] > 0 and d * k <= E_V[prec]:
+    if k > 0 and E_V[prec] > 0 and d <= E_V[prec] / k + float(draw_term(np.float64(delta), np.float64(k), beta, prec)):
         return "conditioned"
     return None
 

@@ -61,11 +61,11 @@ def test_sampled_link_parity_at_bench_sizes(dims, prec, start, beta):
                                np.arange(0, 2 * dims[0]), V - 1 - np.arange(0, 2 * dims[0])])
         cand = np.unique(cand[par_of(cand) == p])[: n_sample + 2 * dims[0]]
         for s in cand:
-            u, tr, mg, k = oracle.heatbath_link(dims, before, beta, seed, 2, int(s), mu, mode, return_k=True)
+            u, tr, mg, k, dl = oracle.heatbath_link(dims, before, beta, seed, 2, int(s), mu, mode, return_k=True, return_delta=True)
             d = np.abs(after[s, mu].astype(np.float64) - u.astype(np.float64)).max()
             sampled += 1
             if d > TOL[prec]:
-                why = sampled_link_excused(d, mg, k, prec)
+                why = sampled_link_excused(d, mg, k, dl, beta, prec)
                 assert why, (s, mu, d, mg, k)
                 flips += why == "flip"
                 small += why == "conditioned"
@@ -106,13 +106,13 @@ def test_sampled_link_parity_at_32c4_with_auto_draw(prec):
             cand = np.concatenate([rng.integers(0, V, size=1200), [0, V - 1, 31, V - 32]])
             cand = np.unique(cand[par_of(cand) == p])[:400]
             for s in cand:
-                u, tr, mg, k = oracle.heatbath_link(dims, before, beta, seed, 1, int(s), mu, mode, return_k=True)
+                u, tr, mg, k, dl = oracle.heatbath_link(dims, before, beta, seed, 1, int(s), mu, mode, return_k=True, return_delta=True)
                 n_creutz += beta * k < oracle.ALPHA_C
                 n_kp += beta * k >= oracle.ALPHA_C
                 d = np.abs(after[s, mu].astype(np.float64) - u.astype(np.float64)).max()
                 sampled += tr
                 if d > TOL[prec]:
-                    why = sampled_link_excused(d, mg, k, prec)
+                    why = sampled_link_excused(d, mg, k, dl, beta, prec)
                     assert why, (s, mu, d, mg, k)
                     flips += why == "flip"
                     small += why == "conditioned"

@@ -73,11 +73,11 @@ def test_128c3x144_fp32_offsets_beyond_32_bits():
         cand = np.unique(cand[par == p])
         assert len(cand) > 500 and cand.max() * 16 > 2**32
         for s in cand:
-            u, tr, mg, k = oracle.heatbath_link(dims, before, beta, seed, 1, int(s), mu, mode, return_k=True)
+            u, tr, mg, k, dl = oracle.heatbath_link(dims, before, beta, seed, 1, int(s), mu, mode, return_k=True, return_delta=True)
             d = np.abs(after[s, mu].astype(np.float64) - u.astype(np.float64)).max()
             sampled += 1
             if d > 1e-5:
-                why = sampled_link_excused(d, mg, k, prec)
+                why = sampled_link_excused(d, mg, k, dl, beta, prec)
                 assert why, (s, mu, d, mg, k)
                 flips += why == "flip"
                 small += why == "conditioned"

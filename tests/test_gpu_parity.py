@@ -28,11 +28,6 @@ def pkg():
     return p
 
 
-def records(V):
-    """the oracle's per-link accept margin and staple norm, filled by the heat-bath calls"""
-    return np.ones((V, 4)), np.ones((V, 4))
-
-
 def assert_links_equal_within_tol(gpu, ora, prec, what=""):
     """no excuse of any kind (fp64 chains, untouched links)"""
     d = np.abs(gpu.astype(np.float64) - ora.astype(np.float64))
@@ -85,9 +80,9 @@ def test_every_substep_matches_oracle_teacher_forced(pkg, dims, prec):
             lat.substep(beta, sweep, mu, p)
             g = lat.get_links()
             o = L.copy()
-            mg, kn = records(V)
-            oracle.heatbath_substep(dims, o, beta, seed, sweep, mu, p, mode, margin=mg, knorm=kn)
-            pp.compare_links(g, o, dims, prec, [(mu, p)], mg, kn, what=f"mu={mu} p={p}")
+            rec = pp.Records(V)
+            oracle.heatbath_substep(dims, o, beta, seed, sweep, mu, p, mode, **rec.kw)
+            pp.compare_links(g, o, dims, prec, [(mu, p)], rec, beta, what=f"mu={mu} p={p}")
             # only the links of this sub-step changed
             untouched = np.ones((V, 4), bool)
             s = np.arange(V)
@@ -113,9 +108,9 @@ def test_sweep_on_smooth_lattice_matches_oracle(pkg, prec, eps, beta):
     lat.set_seed(77)
     lat.sweep(beta, 3)
     g = lat.get_links()
-    mg, kn = records(oracle.volume(dims))
-    oracle.heatbath_sweep(dims, L, beta, 77, 3, mode, margin=mg, knorm=kn)
-    rep = pp.compare_links(g, L, dims, prec, SWEEP, mg, kn, haar=False)
+    rec = pp.Records(oracle.volume(dims))
+    oracle.heatbath_sweep(dims, L, beta, 77, 3, mode, **rec.kw)
+    rep = pp.compare_links(g, L, dims, prec, SWEEP, rec, beta, haar=False)
     P, Lp = lat.measure()
     pp.check_observables(P, Lp, g, dims, prec, rep, L)
     lat.close()
@@ -163,11 +158,11 @@ def test_fp32_and_fp64_ten_sweeps_16c4_teacher_forced(pkg, prec):
     for i in range(4):
         lat.set_links(L)
         lat.sweep(2.4, i)
-        mg, kn = records(V)
-        oracle.heatbath_sweep(dims, L, 2.4, 100, i, mode, margin=mg, knorm=kn)
+        rec = pp.Records(V)
+        oracle.heatbath_sweep(dims, L, 2.4, 100, i, mode, **rec.kw)
         g = lat.get_links()
         # sweep 0 starts from the Haar-random hot start (small staple norms occur), later ones from beta = 2.4
-        rep = pp.compare_links(g, L, dims, prec, SWEEP, mg, kn, haar=(i == 0), what=f"sweep {i}")
+        rep = pp.compare_links(g, L, dims, prec, SWEEP, rec, 2.4, haar=(i == 0), what=f"sweep {i}")
         flips += rep.flips
         P, Lp = lat.measure()
         pp.check_observables(P, Lp, g, dims, prec, rep, L, what=f"sweep {i}")
@@ -316,11 +311,11 @@ def test_fp32_small_alpha_exercises_the_accurate_refinement(pkg, beta):
         lat.set_links(L)  # teacher-forced: a flipped accept must not feed the next sub-step
         lat.substep(beta, 0, mu, p)
         g = lat.get_links()
-        (mg, kn), tr = records(V), np.zeros((V, 4), np.int32)
-        oracle.heatbath_substep(dims, L, beta, 9, 0, mu, p, mode, margin=mg, trials=tr, knorm=kn)
+        rec, tr = pp.Records(V), np.zeros((V, 4), np.int32)
+        oracle.heatbath_substep(dims, L, beta, 9, 0, mu, p, mode, trials=tr, **rec.kw)
         most = max(most, int(tr.max()))
         # many trials per link at small alpha: each is a chance of a marginal decision
-        pp.compare_links(g, L, dims, prec, [(mu, p)], mg, kn, max_flips=pp.flip_budget(int(tr.sum()), prec),
+        pp.compare_links(g, L, dims, prec, [(mu, p)], rec, beta, max_flips=pp.flip_budget(int(tr.sum()), prec),
                          what=f"mu={mu} p={p}")
     assert most >= 5  # the retry loop really ran
     lat.close()
@@ -471,9 +466,9 @@ def test_creutz_and_auto_draw_match_oracle_teacher_forced(pkg, oracle_draw, dims
         lat.set_links(L)
         lat.substep(beta, 4, mu, p)
         g = lat.get_links()
-        (mg, kn), tr = records(V), np.zeros((V, 4), np.int32)
-        oracle.heatbath_substep(dims, L, beta, 33, 4, mu, p, mode, margin=mg, trials=tr, knorm=kn)
-        pp.compare_links(g, L, dims, prec, [(mu, p)], mg, kn, max_flips=pp.flip_budget(int(tr.sum()), prec),
+        rec, tr = pp.Records(V), np.zeros((V, 4), np.int32)
+        oracle.heatbath_substep(dims, L, beta, 33, 4, mu, p, mode, trials=tr, **rec.kw)
+        pp.compare_links(g, L, dims, prec, [(mu, p)], rec, beta, max_flips=pp.flip_budget(int(tr.sum()), prec),
                          what=f"{method} mu={mu} p={p}")
     lat.close()
 
@@ -557,6 +552,36 @@ def test_run_after_reseed_uses_the_new_seed(pkg, how):
     a.close(); b.close()
 
 
+@pytest.mark.parametrize("graphs", [1, 0])
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", [(16, 8, 8, 4), (32, 32, 32, 32), (6, 4, 10, 2)])
+def test_run_with_tail_overlap_equals_plain_run_bitwise(pkg, dims, prec, graphs):
+    """SU2_OPT_TAIL_OVERLAP: the Polyakov kernel of step i on a second stream beside step i+1, two alternating sets
+    of fused-plaquette partials and loop states, blocks of 8 steps per graph plus a directly enqueued remainder
+    (19 = 2 blocks + 3; 5 = remainder only). Links and every observable equal the plain su2_run's bit for bit."""
+    import torch
+    n1, n2 = 19, 5
+    a, b = pkg.Lattice(dims, prec), pkg.Lattice(dims, prec)
+    b.set_option("tail_overlap", 1)
+    b.set_option("run_graph", graphs)
+    oa = torch.zeros(2 * (n1 + n2), dtype=torch.float64, device="cuda")
+    ob = torch.zeros(2 * (n1 + n2), dtype=torch.float64, device="cuda")
+    for lat, o in ((a, oa), (b, ob)):
+        lat.init("hot", 4)
+        lat.run(2.4, 0, n1, o)
+        lat.run(2.4, n1, n2, o[2 * n1:])
+    torch.cuda.synchronize()
+    assert torch.equal(oa, ob)
+    assert (a.get_links() == b.get_links()).all()
+    # switching the option off again drops the captured block
+    b.set_option("tail_overlap", 0)
+    a.run(2.4, 100, 3, oa)
+    b.run(2.4, 100, 3, ob)
+    torch.cuda.synchronize()
+    assert torch.equal(oa[:6], ob[:6]) and (a.get_links() == b.get_links()).all()
+    a.close(); b.close()
+
+
 def test_set_option_rejects_bad_arguments(pkg):
     lat = pkg.Lattice((4, 4, 4, 4), 32)
     for opt, val in ((7, 1), (pkg.SU2_OPT_OVERLAP, 2), (pkg.SU2_OPT_RUN_GRAPH, -1)):
@@ -616,9 +641,9 @@ def test_batch_equals_single_lattices_bitwise_and_matches_oracle(pkg, oracle_dra
     bat.batch_sweep_measure(betas, 9, out, 0)
     g = bat.get_links()
     V = oracle.volume(dims)
-    mg, kn = records(V)
-    oracle.heatbath_sweep(dims, L, betas[3], seeds[3], 9, mode, margin=mg, knorm=kn)
-    rep = pp.compare_links(g, L, dims, prec, SWEEP, mg, kn, what="batch replica 3")
+    rec = pp.Records(V)
+    oracle.heatbath_sweep(dims, L, betas[3], seeds[3], 9, mode, **rec.kw)
+    rep = pp.compare_links(g, L, dims, prec, SWEEP, rec, betas[3], what="batch replica 3")
     P, Lp = out.cpu().numpy()[6:8]
     pp.check_observables(P, Lp, g, dims, prec, rep, L, what="batch replica 3")
     bat.close()

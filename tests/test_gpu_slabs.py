@@ -85,9 +85,9 @@ def test_slab_substeps_match_oracle_teacher_forced(pkg, slabs, dims, n, prec):
             ring.substep(beta, sweep, mu, p)
             g = ring.get_links()
             o = L.copy()
-            mg, kn = np.ones((V, 4)), np.ones((V, 4))
-            oracle.heatbath_substep(dims, o, beta, seed, sweep, mu, p, mode, margin=mg, knorm=kn)
-            pp.compare_links(g, o, dims, prec, [(mu, p)], mg, kn, what=f"mu={mu} p={p}")  # DESIGN.md 3 [R13], [R13b]
+            rec = pp.Records(V)
+            oracle.heatbath_substep(dims, o, beta, seed, sweep, mu, p, mode, **rec.kw)
+            pp.compare_links(g, o, dims, prec, [(mu, p)], rec, beta, what=f"mu={mu} p={p}")  # DESIGN.md 3 [R13], [R13b]
             untouched = np.ones((V, 4), bool)
             untouched[par == p, mu] = False
             assert (g[untouched] == L[untouched]).all()

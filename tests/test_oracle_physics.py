@@ -550,3 +550,26 @@ def test_correlator_rejects_bad_rmax_and_fp32_mode_tracks_fp64():
     a = oracle.polyakov_correlator(dims, L, 2)
     b = oracle.polyakov_correlator(dims, L.astype(np.float32), 2, "f32")
     assert np.abs(a - b).max() < 2e-7
+
+
+def test_returned_delta_is_one_minus_the_scalar_part_of_the_new_link_times_vbar():
+    """heatbath_*(delta=...) hands out the accepted delta = 1 - x0 of each link ([R13b]'s second amplifier). By
+    [R7] U' = X Vbar^dagger, so the scalar part of U' Vbar is x0: recomputed here from the returned link, the pinned
+    staple and the pinned quaternion product. The degenerate [R8] branch reports delta = 1."""
+    dims = [4, 4, 6, 2]
+    L = workloads.random_links(dims, 23, np.float64)
+    V = oracle.volume(dims)
+    for mu, p in ((1, 0), (2, 1)):
+        before = L.copy()
+        dl = np.full((V, 4), -7.0)
+        oracle.heatbath_substep(dims, L, 1.7, 3, 2, mu, p, delta=dl)
+        sites = np.flatnonzero(dl[:, mu] != -7.0)
+        assert len(sites) == V // 2 and (dl[:, [n for n in range(4) if n != mu]] == -7.0).all()
+        assert (dl[sites, mu] > 0).all() and (dl[sites, mu] < 2).all()
+        for s in sites[::7]:
+            v = oracle.staple(dims, before, int(s), mu)
+            x = oracle.qmul(L[s, mu], v / np.linalg.norm(v))
+            assert abs((1.0 - x[0]) - dl[s, mu]) < 1e-14
+            assert oracle.heatbath_link(dims, before, 1.7, 3, 2, int(s), mu, return_delta=True)[3] == dl[s, mu]
+    Z = workloads.degenerate_staple_links((4, 4, 4, 4), 37, 1)
+    assert oracle.heatbath_link((4, 4, 4, 4), Z, 2.3, 5, 0, 37, 1, return_delta=True)[3] == 1.0

@@ -38,12 +38,21 @@ def test_staple_dependency_geometry_matches_the_oracle(dims):
                 assert not others.any()
 
 
-def _sweep_records(dims, mode, seed=3, beta=2.3):
+BETA = 2.3
+
+
+def _sweep_records(dims, mode, seed=3):
     L = workloads.random_links(dims, 8, oracle.dtype(mode))
-    V = oracle.volume(dims)
-    mg, kn = np.ones((V, 4)), np.ones((V, 4))
-    oracle.heatbath_sweep(dims, L, beta, seed, 0, mode, margin=mg, knorm=kn)
-    return L, mg, kn
+    rec = pp.Records(oracle.volume(dims))
+    oracle.heatbath_sweep(dims, L, BETA, seed, 0, mode, **rec.kw)
+    return L, rec.margin, rec.knorm
+
+
+def R(mg, kn):
+    """Records with hand-set margins / staple norms and a well-conditioned draw (delta = 1)"""
+    rec = pp.Records(len(mg))
+    rec.margin, rec.knorm = mg, kn
+    return rec
 
 
 def test_protocol_verdicts_on_hand_made_deviations():
@@ -51,27 +60,27 @@ def test_protocol_verdicts_on_hand_made_deviations():
     ora, mg, kn = _sweep_records(dims, "f32")
     V = oracle.volume(dims)
     # identical and within-tolerance results are clean
-    assert pp.compare_links(ora, ora, dims, prec, pp.SWEEP, mg, kn).clean
+    assert pp.compare_links(ora, ora, dims, prec, pp.SWEEP, R(mg, kn), BETA).clean
     near = ora + np.float32(3e-6)
-    assert pp.compare_links(near, ora, dims, prec, pp.SWEEP, mg, kn).clean
+    assert pp.compare_links(near, ora, dims, prec, pp.SWEEP, R(mg, kn), BETA).clean
     # an O(1) deviation with a healthy margin and a healthy k has no excuse
     s, mu = 77, 3   # direction 3 is updated last: nothing is downstream of it
     assert mg[s, mu] > 1e-3 and kn[s, mu] > 0.5
     gpu = ora.copy()
     gpu[s, mu] = -gpu[s, mu]
     with pytest.raises(AssertionError, match="no excuse"):
-        pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, mg, kn)
+        pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, R(mg, kn), BETA)
     # the same deviation with a marginal accept decision is one flip ...
     m2 = mg.copy()
     m2[s, mu] = 3e-7
-    r = pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, m2, kn)
+    r = pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, R(m2, kn), BETA)
     assert (r.flips, r.conditioned, r.downstream) == (1, 0, 0)
     # ... two such links exceed the budget of a 2048-link sweep
     gpu2 = gpu.copy()
     gpu2[s + 2, mu] = -gpu2[s + 2, mu]
     m2[s + 2, mu] = 1e-7
     with pytest.raises(AssertionError, match="budget"):
-        pp.compare_links(gpu2, ora, dims, prec, pp.SWEEP, m2, kn)
+        pp.compare_links(gpu2, ora, dims, prec, pp.SWEEP, R(m2, kn), BETA)
     # a flip in an early sub-step excuses what is downstream of it, and only that
     s1, mu1 = 40, 0
     gpu = ora.copy()
@@ -87,12 +96,12 @@ def test_protocol_verdicts_on_hand_made_deviations():
     idx = np.flatnonzero(hit.reshape(-1))
     assert len(idx) > 0
     gpu[idx[0], 1] = -gpu[idx[0], 1]
-    r = pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, m3, kn)
+    r = pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, R(m3, kn), BETA)
     assert (r.flips, r.downstream) == (1, 1)
     far = int(np.flatnonzero(~hit.reshape(-1) & (par.reshape(-1) == 1 - p1))[-1])
     gpu[far, 1] = -gpu[far, 1]
     with pytest.raises(AssertionError, match="no excuse"):
-        pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, m3, kn)
+        pp.compare_links(gpu, ora, dims, prec, pp.SWEEP, R(m3, kn), BETA)
 
 
 def test_conditioning_bound_scales_with_one_over_k_and_with_the_inputs_and_is_fp32_only():
@@ -104,40 +113,69 @@ def test_conditioning_bound_scales_with_one_over_k_and_with_the_inputs_and_is_fp
     k2[s, mu] = 0.04                      # E_V / k = 5e-5
     gpu = ora.copy()
     gpu[s, mu, 1] += np.float32(4e-5)
-    r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k2)
+    r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, R(mg, k2), BETA)
     assert (r.flips, r.conditioned) == (0, 1)
     gpu[s, mu, 1] += np.float32(4e-5)     # 8e-5 > E_V / k: more than 1/k explains
     with pytest.raises(AssertionError, match="no excuse"):
-        pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k2)
+        pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, R(mg, k2), BETA)
     # a well-conditioned link (k = 0.5) may exceed 1e-5 only by what the measured deviation of its inputs explains
     k3 = kn.copy()
     k3[s, mu] = 0.5
     gpu = ora.copy()
     gpu[s, mu, 2] += np.float32(2.5e-5)
     with pytest.raises(AssertionError, match="no excuse"):
-        pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k3)
+        pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, R(mg, k3), BETA)
     # ... one of its inputs, updated earlier in the sweep (direction 0), deviates by 8e-6 (inside tolerance):
     # (E_V + 2 x 8e-6) / 0.5 = 3.6e-5 >= 2.5e-5
     s_in = s                                             # U_0(x): the staple input 'U_nu(x)' with nu = 0
     gpu[s_in, 0, 0] += np.float32(8e-6)
-    r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, mg, k3)
+    r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, R(mg, k3), BETA)
     assert (r.flips, r.conditioned, r.downstream) == (0, 1, 0)
     # the same deviation on a link of direction 3's own sub-step partner (updated later or never read) does not help
     gpu2 = ora.copy()
     gpu2[s, mu, 2] += np.float32(2.5e-5)
     gpu2[(s + 5) % V, 1, 0] += np.float32(8e-6)
     with pytest.raises(AssertionError, match="no excuse"):
-        pp.compare_links(gpu2, ora, dims, 32, pp.SWEEP, mg, k3)
+        pp.compare_links(gpu2, ora, dims, 32, pp.SWEEP, R(mg, k3), BETA)
     # fp64 has no conditioning excuse and a zero flip budget
     o64, m64, k64 = _sweep_records(dims, "f64")
     g64 = o64.copy()
     g64[s, mu, 1] += 1e-11
     k64[s, mu] = 1e-4
     with pytest.raises(AssertionError, match="no excuse"):
-        pp.compare_links(g64, o64, dims, 64, pp.SWEEP, m64, k64)
+        pp.compare_links(g64, o64, dims, 64, pp.SWEEP, R(m64, k64), BETA)
     m64[s, mu] = 1e-13
     with pytest.raises(AssertionError, match="budget"):
-        pp.compare_links(g64, o64, dims, 64, pp.SWEEP, m64, k64)
+        pp.compare_links(g64, o64, dims, 64, pp.SWEEP, R(m64, k64), BETA)
+
+
+def test_draw_radius_term():
+    """A rounding of delta = 1 - x0 reaches the link amplified by |1 - delta| / sqrt(delta (2 - delta)): a link whose
+    oracle delta is 1e-4 (radius 0.014) may deviate by E_D (delta + 1/alpha) / 0.014 ~ 1.3e-5 at alpha = 2.3, not more;
+    the same deviation at delta = 0.5 has no excuse."""
+    dims = (8, 4, 4, 4)
+    ora, mg, kn = _sweep_records(dims, "f32")
+    s, mu = 90, 3
+    rec = R(mg, kn.copy())
+    rec.knorm[s, mu] = 1.0            # alpha = 2.3, staple term 2e-6
+    rec.delta[s, mu] = 1e-4
+    allowed = 2e-6 + float(pp.draw_term(1e-4, 1.0, BETA, 32))
+    assert 1.2e-5 < allowed < 1.6e-5
+    gpu = ora.copy()
+    gpu[s, mu, 2] += np.float32(1.2e-5)
+    r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, rec, BETA)
+    assert (r.flips, r.conditioned) == (0, 1)
+    gpu[s, mu, 2] += np.float32(1e-5)
+    with pytest.raises(AssertionError, match="no excuse"):
+        pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, rec, BETA)
+    rec.delta[s, mu] = 0.5
+    gpu = ora.copy()
+    gpu[s, mu, 2] += np.float32(1.2e-5)
+    with pytest.raises(AssertionError, match="no excuse"):
+        pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, rec, BETA)
+    # x0 -> -1 (delta -> 2) is the same
+    rec.delta[s, mu] = 2 - 1e-4
+    assert pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, rec, BETA).conditioned == 1
 
 
 def test_budgets():
@@ -154,10 +192,10 @@ def test_fp32_oracle_modes_agree_under_the_protocol():
     L = workloads.random_links(dims, 2, np.float32)
     V = oracle.volume(dims)
     a, b = L.copy(), L.copy()
-    mg, kn = np.ones((V, 4)), np.ones((V, 4))
-    oracle.heatbath_sweep(dims, a, 2.3, 4, 1, "f32x")
-    oracle.heatbath_sweep(dims, b, 2.3, 4, 1, "f32", margin=mg, knorm=kn)
-    r = pp.compare_links(a, b, dims, 32, pp.SWEEP, mg, kn)
+    rec = pp.Records(V)
+    oracle.heatbath_sweep(dims, a, BETA, 4, 1, "f32x")
+    oracle.heatbath_sweep(dims, b, BETA, 4, 1, "f32", **rec.kw)
+    r = pp.compare_links(a, b, dims, 32, pp.SWEEP, rec, BETA)
     assert r.flips <= 1
     pp.check_observables(oracle.mean_plaquette(dims, a, "f32x"), oracle.polyakov_loop(dims, a, "f32x"), a, dims, 32,
                          rep=r, ora_links=b)
