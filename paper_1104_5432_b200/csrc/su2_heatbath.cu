@@ -255,7 +255,7 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
 #define HB_MINB_F32 8
 #endif
 #ifndef HB_MINB_F64
-#define HB_MINB_F64 7
+#define HB_MINB_F64 6
 #endif
 template <typename Real>
 struct MinBlocks {
@@ -268,14 +268,13 @@ struct MinBlocks<double> {
 
 // tiled launch: one CTA = 2^LHX x 2^LY x 2^LZ x 2^LT threads of a 4-D tile;
 // grid = (nb0, nb1, nb2*nb3): x fastest, so CTAs are scheduled roughly in memory order.
-// TLOOP: consecutive t-tiles one CTA walks through (kTLoop for the hot-path kernels of large fp32 lattices,
-// where a quarter of the CTA launches and drains is worth 4-5 %; 0 = g.tloop at run time, the ALT kernels).
+// TLOOP: consecutive t-tiles one CTA walks through (kTLoop for the hot-path kernels of large lattices, where a
+// quarter of the CTA launches and drains is worth 4-5 % in fp32 and 2 % in fp64; 0 = g.tloop at run time, the
+// ALT kernels).
 #ifndef HB_TLOOP
 #define HB_TLOOP 4
 #endif
-#ifndef HB_WALK_F64
-#define HB_WALK_F64 0
-#endif
+
 constexpr int kTLoop = HB_TLOOP;
 template <typename Real, int MU, int P, bool MEAS, bool ALT, int LHX, int LY, int LZ, int LT, int TLOOP>
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), (MinBlocks<Real>::value << 7) >> (LHX + LY + LZ + LT))
@@ -363,6 +362,7 @@ __global__ void __launch_bounds__(kBlock)
 
 void choose_tiling(Geom& g, int nrep, int precision)
 {
+    (void)precision;  // both precisions use the same tiling (the fp64 kernels took no walk until r02)
     g.tile = -1;
     g.tloop = 1;
     g.nb[0] = g.nb[1] = g.nb[2] = g.nb[3] = 0;
@@ -382,8 +382,8 @@ void choose_tiling(Geom& g, int nrep, int precision)
         g.nb[1] = (int)nb1;
         g.nb[2] = (int)nb2;
         g.nb[3] = (int)nb3;
-        // walk (see heatbath_tiled_kernel): fp32, first tile shape, and at least 4 CTA waves of 148 x 8 left
-        if (k == 0 && (precision == 32 || HB_WALK_F64) && nb3 % kTLoop == 0 && (uint64_t)g.nb[0] * nb1 * nb2 * (nb3 / kTLoop) >= 4736)
+        // walk (see heatbath_tiled_kernel): first tile shape, and at least 4 CTA waves of 148 x 8 left
+        if (k == 0 && nb3 % kTLoop == 0 && (uint64_t)g.nb[0] * nb1 * nb2 * (nb3 / kTLoop) >= 4736)
             g.tloop = kTLoop;
         g.zmagic = (uint32_t)(((1ull << 32) + nb2 - 1) / nb2);  // unused if nb2 == 1
         return;
@@ -426,12 +426,9 @@ static int launch_substep_t(void* links, const Geom& g, double beta, double creu
     hp.nzt = (uint32_t)(g.nb[2] * (g.nb[3] / g.tloop));
     hp.epart_stride = (uint32_t)(3 * heatbath_ctas(g));
     const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * (g.nb[3] / g.tloop) * nrep));
-    // hot-path kernels: the walk length is a template parameter (1, or kTLoop on the first tile shape in fp32);
+    // hot-path kernels: the walk length is a template parameter (1, or kTLoop on the first tile shape);
     // the ALT kernels read it from g
-#ifndef HB_WALK_F64
-#define HB_WALK_F64 0
-#endif
-    constexpr bool kWalk = !ALT && (sizeof(Real) == 4 || HB_WALK_F64);
+    constexpr bool kWalk = !ALT;
     if (g.tile == 0 && kWalk && g.tloop == kTLoop) {
         launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3],
                                         kWalk ? kTLoop : 0>,
