@@ -15,12 +15,14 @@ Tolerances are BASELINE.json north_star's: every link after one sweep |d| <= 1e-
                      turns the max-norm of d into a bound on the quaternion norm). The link's tolerance is
                          max(TOL, (E_V + 2 S_in) / k),   k = the oracle's staple norm for that link.
                      A second amplifier sits in the draw itself: the vector part of X lives on a sphere of
-                     radius rad = sqrt(delta (2 - delta)) [R7], so a rounding of delta = 1 - x0 (two fp32
-                     evaluations of -(ln R + cos^2 ln R'')/alpha differ by <= E_D (delta + 1/alpha), E_D = 4e-7:
-                     a few ulp of the sum, or the MUFU budget of DESIGN.md 6.2) moves it by that times
-                     |1 - delta| / rad - unbounded as x0 -> +-1, probability ~1e-6 per link. With the oracle's
-                     delta for the link:
-                         tol = max(TOL, (E_V + 2 S_in) / k + E_D (delta + 1/alpha) max(1, |1 - delta| / rad)),
+                     radius rad = sqrt(delta (2 - delta)) [R7], so a change of delta = 1 - x0 moves it by that
+                     times A = max(1, |1 - delta| / rad) - unbounded as x0 -> +-1 (probability ~1e-6 per link).
+                     delta = -(ln R + cos^2 ln R'')/alpha changes for two reasons: alpha = beta k carries the
+                     relative error dv/k of the staple norm (|d delta| = delta dv/k), and two fp32 evaluations
+                     of the logs and the cosine differ by <= E_D (delta + 1/alpha), E_D = 4e-7 (a few ulp of the
+                     sum, or the MUFU budget of DESIGN.md 6.2). With the oracle's delta for the link and
+                     dv = E_V + 2 S_in:
+                         tol = max(TOL, dv/k (1 + delta A) + E_D (delta + 1/alpha) A),
                      north_star's 1e-5 wherever the update is well conditioned (k >= 0.2, clean inputs,
                      rad >~ 0.05), wider only by what the two amplifiers explain. Links that need the wider
                      bound are counted against conditioned_budget().
@@ -118,11 +120,16 @@ class Records:
         return dict(margin=self.margin, knorm=self.knorm, delta=self.delta)
 
 
-def draw_term(delta, k, beta, prec):
-    """E_D (delta + 1/alpha) max(1, |1 - delta| / rad): what a rounding of delta does to the new link"""
-    alpha = np.maximum(beta * k, 1e-30)
+def allowed_deviation(delta, k, beta, s_in, prec):
+    """The per-link bound of [R13b]: dv/k, where dv = E_V + 2 S_in, reaches the link directly (Vbar = v/k) and
+    through alpha = beta k (delta ~ 1/alpha: |d delta| = delta dv/k); the rounding of delta itself is
+    E_D (delta + 1/alpha); and every change of delta is amplified by A = max(1, |1 - delta| / rad)."""
+    k = np.maximum(k, 1e-30)
+    alpha = beta * k
     rad = np.sqrt(np.maximum(delta * (2.0 - delta), 1e-30))
-    return E_D[prec] * (delta + 1.0 / alpha) * np.maximum(1.0, np.abs(1.0 - delta) / rad)
+    amp = np.maximum(1.0, np.abs(1.0 - delta) / rad)
+    dvk = (E_V[prec] + 2.0 * s_in) / k
+    return dvk * (1.0 + delta * amp) + E_D[prec] * (delta + 1.0 / alpha) * amp
 
 
 class Report:
@@ -164,8 +171,7 @@ def compare_links(gpu, ora, dims, prec, substeps, rec=None, beta=None, max_flips
         down = staple_inputs_any(taint, mu) & sel
         flip = b & ~down & (m < FLIP_MARGIN[prec])
         s_in = staple_inputs_sum(dev, mu)
-        kk = np.maximum(k, 1e-30)
-        allowed = (E_V[prec] + 2.0 * s_in) / kk + draw_term(dl[..., mu], kk, beta, prec)
+        allowed = allowed_deviation(dl[..., mu], k, beta, s_in, prec)
         cond = b & ~down & ~flip & (k > 0) & (dd <= allowed) & (E_V[prec] > 0)
         unexplained = b & ~down & ~flip & ~cond
         if unexplained.any():
@@ -195,7 +201,7 @@ def sampled_link_excused(d, margin, k, delta, beta, prec):
     downstream): 'flip' [R13], 'conditioned' [R13b] or None."""
     if margin < FLIP_MARGIN[prec]:
         return "flip"
-    if k > 0 and E_V[prec] > 0 and d <= E_V[prec] / k + float(draw_term(np.float64(delta), np.float64(k), beta, prec)):
+    if k > 0 and E_V[prec] > 0 and d <= float(allowed_deviation(np.float64(delta), np.float64(k), beta, 0.0, prec)):
         return "conditioned"
     return None
 

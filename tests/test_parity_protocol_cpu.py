@@ -110,12 +110,12 @@ def test_conditioning_bound_scales_with_one_over_k_and_with_the_inputs_and_is_fp
     V = oracle.volume(dims)
     s, mu = 90, 3
     k2 = kn.copy()
-    k2[s, mu] = 0.04                      # E_V / k = 5e-5
+    k2[s, mu] = 0.04                      # E_V / k = 5e-5, twice that with the delta = 1 of R(): directly and through alpha
     gpu = ora.copy()
     gpu[s, mu, 1] += np.float32(4e-5)
     r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, R(mg, k2), BETA)
     assert (r.flips, r.conditioned) == (0, 1)
-    gpu[s, mu, 1] += np.float32(4e-5)     # 8e-5 > E_V / k: more than 1/k explains
+    gpu[s, mu, 1] += np.float32(9e-5)     # 1.3e-4 > 1.05e-4: more than 1/k explains
     with pytest.raises(AssertionError, match="no excuse"):
         pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, R(mg, k2), BETA)
     # a well-conditioned link (k = 0.5) may exceed 1e-5 only by what the measured deviation of its inputs explains
@@ -126,7 +126,7 @@ def test_conditioning_bound_scales_with_one_over_k_and_with_the_inputs_and_is_fp
     with pytest.raises(AssertionError, match="no excuse"):
         pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, R(mg, k3), BETA)
     # ... one of its inputs, updated earlier in the sweep (direction 0), deviates by 8e-6 (inside tolerance):
-    # (E_V + 2 x 8e-6) / 0.5 = 3.6e-5 >= 2.5e-5
+    # (E_V + 2 x 8e-6) / 0.5 = 3.6e-5 >= 2.5e-5 (and as much again through alpha)
     s_in = s                                             # U_0(x): the staple input 'U_nu(x)' with nu = 0
     gpu[s_in, 0, 0] += np.float32(8e-6)
     r = pp.compare_links(gpu, ora, dims, 32, pp.SWEEP, R(mg, k3), BETA)
@@ -159,7 +159,7 @@ def test_draw_radius_term():
     rec = R(mg, kn.copy())
     rec.knorm[s, mu] = 1.0            # alpha = 2.3, staple term 2e-6
     rec.delta[s, mu] = 1e-4
-    allowed = 2e-6 + float(pp.draw_term(1e-4, 1.0, BETA, 32))
+    allowed = float(pp.allowed_deviation(1e-4, 1.0, BETA, 0.0, 32))
     assert 1.2e-5 < allowed < 1.6e-5
     gpu = ora.copy()
     gpu[s, mu, 2] += np.float32(1.2e-5)
