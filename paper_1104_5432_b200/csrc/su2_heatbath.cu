@@ -47,12 +47,15 @@ struct SiteIdx {
     int t;   // time slice (a slab's edge slices are also stored to its neighbours)
 };
 
-template <typename Real>
+// STATE: 0 = sweep index and 1/beta are launch parameters, 1 = they come from su2_run's device loop state, 2 = decided at
+// run time by hp.state. The hot-path tiled kernels are instantiated for 0 and 1 (the run-time form costs every
+// launch the ~12 instructions of the other one); the ALT and linear kernels use 2.
+template <int STATE, typename Real>
 __device__ __forceinline__ void run_state(const HbParams<Real>& hp, uint32_t& sweep, Real& inv_beta)
 {
     sweep = hp.sweep;
     inv_beta = hp.inv_beta;
-    if (hp.state) {  // su2_run: the captured graph's parameters are frozen, the loop state is not
+    if (STATE == 1 || (STATE == 2 && hp.state)) {  // su2_run: the captured graph's parameters are frozen, the loop state is not
         double ib;
         ld_run_state(run_state_copy(hp.state), ib, sweep);
         inv_beta = (Real)ib;
@@ -78,7 +81,7 @@ __device__ __forceinline__ uint32_t hb_check(uint32_t idx, uint32_t hoff, uint32
 #endif
 
 // neighbour addressing (row 2) and the 18 loads (row 3, first half) of one site
-template <typename Real, int MU, int P>
+template <typename Real, int MU, int P, int STATE>
 __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const HbParams<Real>& hp, Staple18<Real>& q,
                                           uint32_t& sweep, Real& inv_beta, uint32_t hoff, int* __restrict__ err)
 {
@@ -115,7 +118,7 @@ __device__ __forceinline__ SiteIdx load18(const Geom& g, const Site& c, const Hb
         const uint32_t h_upnu = HB_CK(h + d.up[nu]);
         q.b[2] = DEP_MU ? ldq_dep(o_mu + h_upnu) : ldq(o_mu + h_upnu);  // U_mu(x+nu), largest nu
     }
-    run_state(hp, sweep, inv_beta);
+    run_state<STATE>(hp, sweep, inv_beta);
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         const int nu = i + (i >= MU ? 1 : 0);
@@ -228,7 +231,7 @@ __device__ __forceinline__ Real update_link(const Staple18<Real>& q, const SiteI
     return MEAS ? u.a0 * w.a0 - u.a1 * w.a1 - u.a2 * w.a2 - u.a3 * w.a3 : (Real)0;  // 1/2 Tr(U' w)
 }
 
-template <typename Real, int MU, int P, bool MEAS, bool ALT>
+template <typename Real, int MU, int P, bool MEAS, bool ALT, int STATE>
 __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, const HbParams<Real>& hp, uint32_t rep,
                                               int* __restrict__ err)
 {
@@ -239,7 +242,7 @@ __device__ __forceinline__ Real heatbath_site(const Geom& g, const Site& c, cons
     Staple18<Real> q;
     RepCtx rc = {0u, 0u, hp.rk.k[0], hp.rk.k[1]};
     if (ALT) rc = {rep, rep * hp.rep_stride, hp.rk.k[0], hp.rk.k[1]};
-    const SiteIdx ix = load18<Real, MU, P>(g, c, hp, q, sweep, inv_beta, rc.hoff, err);
+    const SiteIdx ix = load18<Real, MU, P, STATE>(g, c, hp, q, sweep, inv_beta, rc.hoff, err);
     if (ALT && hp.reps) {  // batched launch: this replica's coupling and seed
         const RepParams rp = hp.reps[rep];
         inv_beta = (Real)rp.inv_beta;
@@ -276,7 +279,7 @@ struct MinBlocks<double> {
 #endif
 
 constexpr int kTLoop = HB_TLOOP;
-template <typename Real, int MU, int P, bool MEAS, bool ALT, int LHX, int LY, int LZ, int LT, int TLOOP>
+template <typename Real, int MU, int P, bool MEAS, bool ALT, int LHX, int LY, int LZ, int LT, int TLOOP, int STATE>
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), (MinBlocks<Real>::value << 7) >> (LHX + LY + LZ + LT))
     heatbath_tiled_kernel(const Geom g, const HbParams<Real> hp, int* __restrict__ err)
 {
@@ -294,10 +297,11 @@ __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT), (MinBlocks<Real>::v
     if (ALT) c.t += g.t_lo;  // slab: the grid covers the interior slices only
     Real e = 0;
     if (TLOOP == 1) {
-        e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err);
+        e = heatbath_site<Real, MU, P, MEAS, ALT, STATE>(g, c, hp, rep, err);
     } else {
 #pragma unroll 1
-        for (int it = 0; it < tloop; ++it, c.t += 1 << LT) e += heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, rep, err);
+        for (int it = 0; it < tloop; ++it, c.t += 1 << LT)
+            e += heatbath_site<Real, MU, P, MEAS, ALT, STATE>(g, c, hp, rep, err);
     }
     if (MEAS) {  // one fp64 partial per CTA, fixed order
         __shared__ double red[kBlock / 32];
@@ -323,7 +327,7 @@ __global__ void __launch_bounds__(kBlock)
         c.y = (int)(q - q2 * (uint32_t)g.n[1]);
         c.t = (int)(q2 / (uint32_t)g.n[2]);
         c.z = (int)(q2 - (uint32_t)c.t * (uint32_t)g.n[2]);
-        e = heatbath_site<Real, MU, P, MEAS, ALT>(g, c, hp, blockIdx.y, err);  // grid y = replica
+        e = heatbath_site<Real, MU, P, MEAS, ALT, 2>(g, c, hp, blockIdx.y, err);  // grid y = replica
     }
     if (MEAS) {
         __shared__ double red[kBlock / 32];
@@ -426,25 +430,31 @@ static int launch_substep_t(void* links, const Geom& g, double beta, double creu
     hp.nzt = (uint32_t)(g.nb[2] * (g.nb[3] / g.tloop));
     hp.epart_stride = (uint32_t)(3 * heatbath_ctas(g));
     const dim3 grid((unsigned)g.nb[0], (unsigned)g.nb[1], (unsigned)(g.nb[2] * (g.nb[3] / g.tloop) * nrep));
-    // hot-path kernels: the walk length is a template parameter (1, or kTLoop on the first tile shape);
-    // the ALT kernels read it from g
-    constexpr bool kWalk = !ALT;
-    if (g.tile == 0 && kWalk && g.tloop == kTLoop) {
-        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3],
-                                        kWalk ? kTLoop : 0>,
-                  grid, dim3(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3])), st, overlap, g, hp,
-                  err);
-    } else if (g.tile == 0) {
-        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[0][0], kTiles[0][1], kTiles[0][2], kTiles[0][3],
-                                        ALT ? 0 : 1>,
-                  grid, dim3(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3])), st, overlap, g, hp,
-                  err);
-    } else if (g.tile == 1) {
-        launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[1][0], kTiles[1][1], kTiles[1][2], kTiles[1][3],
-                                        ALT ? 0 : 1>,
-                  grid, dim3(1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3])), st, overlap, g, hp,
-                  err);
+    // hot-path kernels: the walk length (1, or kTLoop on the first tile shape) and the source of the loop state are
+    // template parameters; the ALT kernels read both at run time
+    const dim3 block0(1 << (kTiles[0][0] + kTiles[0][1] + kTiles[0][2] + kTiles[0][3]));
+    const dim3 block1(1 << (kTiles[1][0] + kTiles[1][1] + kTiles[1][2] + kTiles[1][3]));
+#define SU2_TILED(K_, TL_, ST_)                                                                                       \
+    launch_ex(heatbath_tiled_kernel<Real, MU, P, MEAS, ALT, kTiles[K_][0], kTiles[K_][1], kTiles[K_][2], kTiles[K_][3], \
+                                    TL_, ST_>,                                                                        \
+              grid, K_ == 0 ? block0 : block1, st, overlap, g, hp, err)
+    if constexpr (ALT) {
+        if (g.tile == 0) SU2_TILED(0, 0, 2);
+        else if (g.tile == 1) SU2_TILED(1, 0, 2);
     } else {
+        if (g.tile == 0 && g.tloop == kTLoop) {
+            if (state) SU2_TILED(0, kTLoop, 1);
+            else SU2_TILED(0, kTLoop, 0);
+        } else if (g.tile == 0) {
+            if (state) SU2_TILED(0, 1, 1);
+            else SU2_TILED(0, 1, 0);
+        } else if (g.tile == 1) {
+            if (state) SU2_TILED(1, 1, 1);
+            else SU2_TILED(1, 1, 0);
+        }
+    }
+#undef SU2_TILED
+    if (g.tile < 0) {
         launch_ex(heatbath_linear_kernel<Real, MU, P, MEAS, ALT>, dim3((unsigned)heatbath_ctas(g), (unsigned)nrep),
                   dim3(kBlock), st, overlap, g, hp, err);
     }
