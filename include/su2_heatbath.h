@@ -47,6 +47,7 @@ extern "C" {
 #define SU2_EALLOC 2  /* device allocation failed */
 #define SU2_ECUDA 3   /* CUDA runtime error; sticky, message via su2_last_error */
 #define SU2_ESTATE 4  /* sweep or measurement before su2_init / su2_set_links */
+#define SU2_ETOOBIG 5 /* su2_mean_plaquette_noalloc only: lattice larger than its static scratch serves */
 
 #define SU2_START_COLD 0
 #define SU2_START_HOT 1
@@ -291,6 +292,25 @@ SU2_API int su2_slab_polyakov(su2_lattice* lat, const void* dev_prev, void* dev_
 SU2_API int su2_ipc_export(su2_lattice* lat, void* handle64);
 SU2_API int su2_ipc_open(const void* handle64, void** dev_ptr);
 SU2_API int su2_ipc_close(void* dev_ptr);
+
+/* Row 7 ([R10]) WITHOUT ANY ALLOCATION: for callers that cannot call cudaMalloc - code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it. No handle (creating one allocates): the caller passes the
+ * configuration and the destination, the call enqueues the plaquette kernel and a final sum on cuda_stream (a
+ * cudaStream_t, may be 0) and calls no cudaMalloc, cudaFree or allocating library routine.
+ *   dev_links [device] a configuration in DEVICE layout (see top: 8 arrays [p][mu] of V/2 quaternions of the
+ *             precision; what su2_device_links returns / what a caller-owned buffer of a handle holds), 32-byte aligned;
+ *   dev_out   [device] receives the mean plaquette (one double) when the stream reaches it. Asynchronous.
+ * The per-CTA partial sums - library-allocated per handle everywhere else - live in ONE file-scope static device
+ * array of 2^18 doubles (2 MiB, held by every GPU that loads the library until exit), which serves lattices of up to
+ * SU2_NOALLOC_MAX_SITES = 2^25 sites (64^4 = 2^24). All calls share it: calls that can overlap on the GPU (different
+ * streams, no ordering between them) race and give wrong results; calls on one stream, or otherwise ordered, are safe.
+ * Nothing in it has to start at zero (each call writes every partial it reads), so it is never cleared.
+ * Same kernels, same fixed reduction order as su2_mean_plaquette: the same bits for the same configuration.
+ * Errors: SU2_EARG (NULL or misaligned pointer, bad extents or precision), SU2_ETOOBIG (V > SU2_NOALLOC_MAX_SITES;
+ * nothing is launched), SU2_ECUDA (launch failure). */
+#define SU2_NOALLOC_MAX_SITES (1u << 25)
+SU2_API int su2_mean_plaquette_noalloc(const void* dev_links, int Nx, int Ny, int Nz, int Nt, int precision,
+                                       void* cuda_stream, double* dev_out);
 
 /* Measurement support: memory bandwidth of the current device with the
  * access shape of the path - 128-bit loads, unit stride across a warp, every SM busy, no arithmetic - over a

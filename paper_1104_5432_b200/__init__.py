@@ -17,7 +17,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsu2hb.so")
 
-SU2_OK, SU2_EARG, SU2_EALLOC, SU2_ECUDA, SU2_ESTATE = 0, 1, 2, 3, 4
+SU2_OK, SU2_EARG, SU2_EALLOC, SU2_ECUDA, SU2_ESTATE, SU2_ETOOBIG = 0, 1, 2, 3, 4, 5
+SU2_NOALLOC_MAX_SITES = 1 << 25
 SU2_START_COLD, SU2_START_HOT = 0, 1
 SU2_DRAW_KP, SU2_DRAW_AUTO, SU2_DRAW_CREUTZ = 0, 1, 2
 SU2_ALPHA_C = 1.6847
@@ -67,6 +68,7 @@ _SIGNATURES = {
     "su2_ipc_export": (C.c_int, [C.c_void_p, C.c_void_p]),
     "su2_ipc_open": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p)]),
     "su2_ipc_close": (C.c_int, [C.c_void_p]),
+    "su2_mean_plaquette_noalloc": (C.c_int, [C.c_void_p] + [C.c_int] * 5 + [C.c_void_p, C.c_void_p]),
     "su2_bandwidth_probe": (C.c_int, [C.c_size_t, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_double),
                                       C.POINTER(C.c_double)]),
     "su2_launch_count": (C.c_uint64, [C.c_void_p]),
@@ -239,6 +241,12 @@ def su2_set_links(h, host_array):
 
 def su2_synchronize(h):
     _check(lib().su2_synchronize(h), h)
+
+
+def su2_mean_plaquette_noalloc(dev_links_ptr, Nx, Ny, Nz, Nt, precision, dev_out_ptr, cuda_stream=0):
+    """Mean plaquette of a device-layout configuration into *dev_out_ptr; allocates nothing (static scratch)."""
+    _check(lib().su2_mean_plaquette_noalloc(C.c_void_p(dev_links_ptr), Nx, Ny, Nz, Nt, precision,
+                                            C.c_void_p(cuda_stream), C.c_void_p(dev_out_ptr)))
 
 
 def su2_bandwidth_probe(nbytes, passes, mode=SU2_PROBE_READ, cuda_stream=0):

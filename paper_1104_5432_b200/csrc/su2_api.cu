@@ -836,6 +836,28 @@ extern "C" int su2_ipc_close(void* dev_ptr)
     return SU2_OK;
 }
 
+extern "C" int su2_mean_plaquette_noalloc(const void* dev_links, int Nx, int Ny, int Nz, int Nt, int precision,
+                                          void* cuda_stream, double* dev_out)
+{
+    if (!dev_links || !dev_out || ((uintptr_t)dev_links & 31) || !valid_dims(Nx, Ny, Nz, Nt, precision)) return SU2_EARG;
+    if ((uint64_t)Nx * Ny * Nz * Nt > SU2_NOALLOC_MAX_SITES) return SU2_ETOOBIG;
+    Geom g = {};  // as create_impl fills it for a whole lattice
+    g.n[0] = Nx; g.n[1] = Ny; g.n[2] = Nz; g.n[3] = Nt;
+    g.nxh = Nx / 2;
+    g.sy = g.nxh;
+    g.sz = g.nxh * Ny;
+    g.st = g.nxh * Ny * Nz;
+    g.vh = (uint32_t)((uint64_t)Nx * Ny * Nz * Nt / 2);
+    g.wup[0] = -(g.nxh - 1);
+    g.wup[1] = -(Ny - 1) * g.sy;
+    g.wup[2] = -(Nz - 1) * g.sz;
+    g.wup[3] = -(Nt - 1) * g.st;
+    g.t_lo = 0;
+    g.nt_upd = Nt;
+    choose_tiling(g, 1, precision);
+    return launch_plaquette_noalloc(dev_links, g, precision, dev_out, (cudaStream_t)cuda_stream);
+}
+
 extern "C" int su2_bandwidth_probe(size_t bytes, int passes, int mode, void* cuda_stream, double* gbs_out,
                                    double* us_per_pass_out)
 {
@@ -859,6 +881,7 @@ extern "C" const char* su2_strerror(int code)
         case SU2_EALLOC: return "device allocation failed";
         case SU2_ECUDA: return "CUDA runtime error";
         case SU2_ESTATE: return "bad state: lattice not initialised";
+        case SU2_ETOOBIG: return "lattice exceeds SU2_NOALLOC_MAX_SITES, the static scratch of su2_mean_plaquette_noalloc";
         default: return "unknown error code";
     }
 }

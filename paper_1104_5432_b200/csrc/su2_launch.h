@@ -99,6 +99,9 @@ int launch_polyakov_correlator(const Geom& g, const Scratch& sc, int rmax, doubl
 int launch_to_device_layout(const void* canonical, void* links, const Geom& g, int precision, cudaStream_t st);
 int launch_to_canonical(const void* links, void* canonical, const Geom& g, int precision, cudaStream_t st);
 
+// no-allocation mean plaquette (su2_measure.cu): partials in a file-scope static __device__ array; returns an SU2_* code
+int launch_plaquette_noalloc(const void* links, const Geom& g, int precision, double* dev_dst, cudaStream_t st);
+size_t noalloc_max_partials();
 // su2_probe.cu: returns an SU2_* code
 int run_bandwidth_probe(size_t bytes, int passes, int mode, cudaStream_t st, double* gbs_out, double* us_per_pass_out);
 

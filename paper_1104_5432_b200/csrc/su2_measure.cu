@@ -570,4 +570,73 @@ int launch_to_canonical(const void* links, void* canonical, const Geom& g, int p
     return 1;
 }
 
+// ------------------------------------------------------------------ no-allocation mean plaquette
+// su2_mean_plaquette_noalloc (include/su2_heatbath.h): row 7 for callers that cannot call cudaMalloc (code under
+// CUDA graph capture, tight serving loops, harnesses that forbid it). The per-CTA partial sums - the scratch of the
+// plaquette kernels, library-allocated per handle everywhere else - live in this file-scope array instead: every GPU
+// that loads the library holds its 2 MiB until exit. One partial per 128 (tiled) or 256 (linear) sites, so it
+// serves lattices of up to kNoAllocMaxPartials * 128 = 2^25 sites (64^4 is 2^24).
+// All calls share the array: it keeps the previous call's partials, none of which is read (every launch writes
+// the n partials its final sum reads, nothing needs to start at zero); calls that overlap on the GPU race.
+constexpr size_t kNoAllocMaxPartials = size_t(1) << 18;
+static __device__ __align__(256) double g_noalloc_partials[kNoAllocMaxPartials];
+
+// variant of final_sum_kernel that names the static array itself (device code may; host code needs the address)
+__global__ void __launch_bounds__(1024) final_sum_static_kernel(size_t n, double scale, double* __restrict__ dst)
+{
+    __shared__ double red[32];
+    double acc = 0.0;
+    for (size_t i = threadIdx.x; i < n; i += 1024) acc += g_noalloc_partials[i];
+    const double tot = block_sum(acc, red);
+    if (threadIdx.x == 0) dst[0] = tot * scale;
+}
+
+// In host code `g_noalloc_partials` is a host-side stand-in, not a device address: the plaquette kernels take the
+// address cudaGetSymbolAddress returns, looked up once per device with that device current.
+static double* noalloc_partials_of_current_device(cudaError_t* ce)
+{
+    constexpr int kMaxDevices = 64;
+    static double* ptr[kMaxDevices] = {};
+    int dev = -1;
+    *ce = cudaGetDevice(&dev);
+    if (*ce != cudaSuccess) return nullptr;
+    if (dev < 0 || dev >= kMaxDevices) {
+        *ce = cudaErrorInvalidDevice;
+        return nullptr;
+    }
+    if (!ptr[dev]) {
+        double* p = nullptr;
+        *ce = cudaGetSymbolAddress((void**)&p, g_noalloc_partials);
+        if (*ce != cudaSuccess) return nullptr;
+        ptr[dev] = p;
+    }
+    return ptr[dev];
+}
+
+size_t noalloc_max_partials() { return kNoAllocMaxPartials; }
+
+// returns an SU2_* code (0 ok, 3 CUDA error, 5 too large); enqueues 2 kernels on `st`, allocates nothing
+int launch_plaquette_noalloc(const void* links, const Geom& g, int precision, double* dev_dst, cudaStream_t st)
+{
+    // partials the launch will write (same formula as launch_plaquette_t)
+    const size_t need = g.tile >= 0 ? 2 * (size_t)g.nb[0] * g.nb[1] * g.nb[2] * g.nb[3]
+                                    : 2 * (size_t)blocks_for((uint64_t)g.st * g.nt_upd);
+    if (need > kNoAllocMaxPartials) return 5;
+    cudaError_t ce = cudaSuccess;
+    Scratch sc = {};
+    sc.partials = noalloc_partials_of_current_device(&ce);
+    if (!sc.partials) {
+        cudaGetLastError();
+        return 3;
+    }
+    sc.n_partials = kNoAllocMaxPartials;
+    size_t n = 0;
+    if (precision == 32)
+        launch_plaquette_t<float>(links, g, sc, &n, st);
+    else
+        launch_plaquette_t<double>(links, g, sc, &n, st);
+    final_sum_static_kernel<<<1, 1024, 0, st>>>(n, 1.0 / (6.0 * 2.0 * (double)g.vh), dev_dst);
+    return cudaGetLastError() == cudaSuccess ? 0 : 3;
+}
+
 }  // namespace su2
