@@ -65,11 +65,14 @@ __global__ void __launch_bounds__(kBlock)
 // serves 56 % of the reads, L2 -> SM traffic falls by 30 %, yet 347 against 302 us at 64^4 fp32), and host-resolved
 // array bases with 32-bit indices and an fp32 per-site sum (11 % fewer instructions, 343 us): the kernel is
 // bound by the latency of its load batches at 29 resident warps, neither by L2 bandwidth nor by issue slots.
+// (Repeated with the round-1 pointer arithmetic, in case the parameter-table lookups had cost the first attempt:
+// L2 -> SM traffic 3.62 -> 2.53 GB, 301 -> 313 us. Not L2-bound.) fp64: 6 resident CTAs (80 registers) instead of 4
+// (126): 553 -> 523 us at 64^4 = 0.63 of the copy peak.
 #ifndef PLAQ_MINB_F32
 #define PLAQ_MINB_F32 8
 #endif
 #ifndef PLAQ_MINB_F64
-#define PLAQ_MINB_F64 4
+#define PLAQ_MINB_F64 6
 #endif
 template <typename Real, int LHX, int LY, int LZ, int LT>
 __global__ void __launch_bounds__(1 << (LHX + LY + LZ + LT),
