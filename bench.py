@@ -635,6 +635,13 @@ def main():
         t = torch.tensor([ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
+        # every timed region is over: release the other ranks now (rank 0 alone goes on to the other metric points,
+        # e2e and the CPU baseline - minutes during which they would sit in a collective)
+        dist.barrier()
+        dist.destroy_process_group()
+        if rank != 0:
+            sampler.stop()
+            return 0
     value = world * w.links * args.steps / (ms * 1e-3)
 
     # L2 roofline denominator: read bandwidth of a 64 MiB buffer - the size of the
@@ -697,9 +704,6 @@ def main():
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": slab.describe(prec) + f" ({sec:.1f} s)"}
     sampler.stop()
-    if world > 1:
-        dist.barrier()
-        dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(line))
     return 0

@@ -649,6 +649,39 @@ def test_batch_equals_single_lattices_bitwise_and_matches_oracle(pkg, oracle_dra
     bat.close()
 
 
+@pytest.mark.parametrize("dims,R,why", [
+    ((32, 4, 64, 64), 40, "2048 z-t tiles of the first shape x 40 replicas exceed grid z: second tile shape"),
+    ((16, 4, 64, 128), 33, "first shape does not divide Nx/2 = 8, second gives 2048 x 33 > 65535: linear launch"),
+])
+def test_batch_falls_back_to_another_launch_shape_instead_of_failing(pkg, dims, R, why):
+    """A batch carries the replica in grid z next to the z-t tiles; where that exceeds the grid limit, create picks
+    the next tile shape or the linear launch (round 1 returned SU2_EARG). Draws are keyed by the site, so the links
+    equal those of single-lattice handles (which use another launch shape) bit for bit."""
+    import torch
+    bat = pkg.Lattice(dims, 32, replicas=R)
+    seeds = [500 + r for r in range(R)]
+    betas = [2.2 + 0.01 * r for r in range(R)]
+    bat.batch_init("hot", seeds)
+    out = torch.zeros(2 * R * 2, dtype=torch.float64, device="cuda")
+    for i in range(2):
+        bat.batch_sweep_measure(betas, i, out, i)
+    torch.cuda.synchronize()
+    o = out.cpu().numpy().reshape(2, R, 2)
+    for r in (0, R // 2, R - 1):
+        one = pkg.Lattice(dims, 32)
+        one.init("hot", seeds[r])
+        o1 = torch.zeros(4, dtype=torch.float64, device="cuda")
+        for i in range(2):
+            one.sweep_measure(betas[r], i, o1, i)
+        torch.cuda.synchronize()
+        bat.select(r)
+        assert (bat.get_links() == one.get_links()).all(), (r, why)
+        # the fused-plaquette partials follow the launch shape: same value to rounding, not the same bits
+        assert np.abs(o[:, r, :] - o1.cpu().numpy().reshape(2, 2)).max() < 2e-7
+        one.close()
+    bat.close()
+
+
 def test_batch_argument_checks(pkg):
     import torch
     with pytest.raises(pkg.SU2Error):
