@@ -399,6 +399,29 @@ def time_e2e(pkg, torch, w, prec, beta, steps, warmup, seed):
             "what": "su2_set_links(pinned host) + su2_heatbath_sweep_measure + su2_get_links(pinned host) + 16 B of observables"}
 
 
+def cpu_fig1(fig1):
+    """The CPU side of the paper's Fig. 1 job ("the serial code in one CPU core"), part of
+    the cpu_baseline leg: the oracle on the same job at 32^4 in fp32 - random start, then heat-bath iterations with the
+    plaquette after each - timed over 3 iterations and scaled to the 100 of the figure (the full job is ~2.5
+    minutes of one core)."""
+    import oracle
+    dims, n_cpu = (32, 32, 32, 32), 3
+    t0 = time.perf_counter()
+    L = oracle.init(dims, "hot", 1, "f32")
+    t_init = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    P = 0.0
+    for i in range(n_cpu):
+        oracle.heatbath_sweep(dims, L, 6.0, 1, i, "f32")
+        P = oracle.mean_plaquette(dims, L, "f32")
+    t_iter = (time.perf_counter() - t0) / n_cpu
+    gpu = next(f for f in fig1 if f["L"] == 32 and f["precision"] == 32)
+    return {"seconds_scaled_to_100_iterations": t_init + 100 * t_iter, "seconds_per_iteration": t_iter,
+            "init_seconds": t_init, "iterations_timed": n_cpu, "cores": 1, "kind": "oracle", "plaquette_after_3": P,
+            "gpu_seconds_same_job": gpu["seconds"], "ratio": (t_init + 100 * t_iter) / gpu["seconds"],
+            "note": "context only (the paper quotes > 200x for 2 GTX 480 over one i7-920 core, PAPER.md:95)"}
+
+
 # ------------------------------------------------------------------------------- oracle
 class OracleSlab:
     """The oracle as it stands (gcc -O2, serial, one host core) on a BOUNDED sample of the
@@ -703,6 +726,7 @@ def main():
         v, sec, n, _, _ = slab.step()
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": slab.describe(prec) + f" ({sec:.1f} s)"}
+        line["cpu_baseline"]["fig1_32^4_fp32"] = cpu_fig1(line["aux"]["fig1_init_100_sweeps_plaquette_beta6"])
     sampler.stop()
     if rank == 0:
         print(json.dumps(line))
