@@ -9,7 +9,8 @@ Tolerances are BASELINE.json north_star's: every link after one sweep |d| <= 1e-
   conditioned [R13b] (fp32 only) the draw divides the staple sum v by its norm k (Vbar = v/k, [R7]), so a
                      perturbation dv of the staple reaches the new link as |dv|/k. dv has two sources,
                      both known to the harness: the rounding of the 12 fp32 products of the staple,
-                     |dv| <= E_V = 2e-6 (measured: max |d| k = 1.4e-6 over 1.3e7 links, profiles/r02a.md),
+                     |dv| <= E_V = 2e-6 (measured: max |d| k = 2.1e-6 over the links with k < 0.5 of 1.26e7, which
+                     includes the (1 + delta A) factor below; profiles/r02a.md),
                      and the deviations the 18 input links already carry when earlier sub-steps of the
                      same sweep wrote them, |dv| <= 2 S_in, S_in = the sum of their measured |d| (the 2
                      turns the max-norm of d into a bound on the quaternion norm). The link's tolerance is
