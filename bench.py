@@ -319,6 +319,28 @@ def time_aux(pkg, torch, workloads):
         out[f"C2_16^3x4_batch{R}"] = {"us_per_round": dt / n * 1e6, "value": R * w.links * n / dt, "unit": UNIT,
                                       "replicas": R, "precision": 32, "rounds": n}
         bat.close()
+    # ... and the paper's benchmark shape: four 32^4 lattices stepped by the launches of one (a 32^4 launch is 3.5 CTA
+    # waves and latency-bound; four of them are 14 waves)
+    w3 = workloads.BY_NAME["C3_32^4"]
+    R, n = 4, 100
+    bat = pkg.Lattice(w3.dims, 32, replicas=R)
+    bat.batch_init(w3.start, [w3.seed + r for r in range(R)])
+    obs = torch.zeros(2 * R * n, dtype=torch.float64, device=bat.device)
+    for i in range(5):
+        bat.batch_sweep_measure([6.0] * R, i, obs, i)
+    bat.synchronize()
+    time.sleep(2.0)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for i in range(n):
+        bat.batch_sweep_measure([6.0] * R, 5 + i, obs, i)
+    b.record()
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / n
+    out["C3_32^4_fp32_batch4"] = {"ms_per_round": ms, "value": R * w3.links / ms * 1e3, "unit": UNIT, "replicas": R,
+                                  "precision": 32, "rounds": n}
+    bat.close()
+    torch.cuda.empty_cache()
     # time slabs (S8(f) NEXT-4) with every slab on this ONE GPU: the slabs' kernels of a sub-step run one
     # after the other, so the sweep time is the sum over slabs - what the split costs in kernel time
     # (ALT kernels, peer stores, no launch overlap), not a multi-GPU number
