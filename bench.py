@@ -235,6 +235,7 @@ def time_workload(pkg, torch, w, prec, beta, steps, warmup, seed, sampler=None, 
     # extra (not the headline): the same `steps` steps as ONE su2_run call - the step captured as
     # a CUDA graph and replayed, no host work per step (matters on small lattices)
     time.sleep(COOL_DOWN_S)  # same power state as the burst leg started from
+    lat.set_option("tail_overlap", 0)  # (the default is automatic; both settings are timed explicitly)
     lat.run(beta, 1 << 20, min(warmup, steps), obs)  # captures the graph
     torch.cuda.synchronize()
     s2, e2 = ev(), ev()

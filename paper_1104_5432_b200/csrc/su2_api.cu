@@ -30,7 +30,8 @@ struct su2_lattice {
     cudaEvent_t run_ev_in, run_ev_out;
     cudaGraphExec_t run_exec;
     bool run_graphs;   // su2_run replays a captured CUDA graph (su2_set_option SU2_OPT_RUN_GRAPH)
-    bool tail_overlap; // su2_run: the Polyakov kernel of a step runs beside the next step (SU2_OPT_TAIL_OVERLAP)
+    int tail_overlap;  // su2_run: the Polyakov kernel of a step runs beside the next step (SU2_OPT_TAIL_OVERLAP):
+                       // 0 off, 1 on, -1 (default) automatic - see tail_overlap_on()
     cudaStream_t tail_stream;
     cudaEvent_t ev_fork, ev_join;
     int run_block;     // steps per captured graph (1, or kRunBlock with tail overlap)
@@ -157,6 +158,7 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, int nrep, 
     lat->last_substep = -1;
     lat->pdl = true;
     lat->run_graphs = true;
+    lat->tail_overlap = -1;
     lat->stream = (cudaStream_t)stream;
     lat->owns_links = !external;
     lat->links = dev_links;
@@ -273,7 +275,7 @@ extern "C" int su2_set_option(su2_lattice* lat, int option, int value)
     switch (option) {
         case SU2_OPT_OVERLAP: lat->pdl = value != 0; break;
         case SU2_OPT_RUN_GRAPH: lat->run_graphs = value != 0; break;
-        case SU2_OPT_TAIL_OVERLAP: lat->tail_overlap = value != 0; break;
+        case SU2_OPT_TAIL_OVERLAP: lat->tail_overlap = value != 0 ? 1 : 0; break;
         default: return fail(lat, SU2_EARG, "su2_set_option: unknown option");
     }
     drop_run_graph(lat);  // the captured step was built with the other setting
@@ -452,6 +454,14 @@ extern "C" int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_
     return SU2_OK;
 }
 
+// Automatic choice: on wherever a sub-step is a few CTA waves - every lattice that does not take
+// the walk (g.tloop == 1: below ~5 M sites) - where it is worth 5-23 % of a step and never costs; off on the large
+// lattices, where forcing sub-step (3,0) behind two predecessors costs 4 %.
+static bool tail_overlap_on(const su2_lattice* lat)
+{
+    return lat->tail_overlap < 0 ? lat->g.tloop == 1 : lat->tail_overlap != 0;
+}
+
 // Steps of su2_run on stream `st`, every per-step quantity read from a device RunState.
 // Plain mode (tail_st == NULL): 8 sub-steps + the Polyakov kernel with the step tail, all on `st`, one loop state.
 // Tail overlap: the Polyakov kernel reads only U_t, which the next step does not write before its
@@ -459,8 +469,11 @@ extern "C" int su2_heatbath_sweep_measure(su2_lattice* lat, double beta, uint32_
 // before the next (3,0). What the two then touch at the same time alternates between two sets by step parity:
 // the fused-plaquette partials (written by (1,1), (2,1), (3,1), read by the tail) and the loop state (read by the
 // sub-steps, advanced - by 2 - by the tail). Same kernels on the same inputs: bit-identical results.
-static const int kRunBlock = 8;  // steps per captured graph with tail overlap (graph launches serialise: the last
-                                 // tail of a block is not overlapped)
+#ifndef SU2_RUN_BLOCK
+#define SU2_RUN_BLOCK 16
+#endif
+static const int kRunBlock = SU2_RUN_BLOCK;  // steps per captured graph with tail overlap (graph launches serialise: the last
+                                              // tail of a block is not overlapped; 4 / 8 / 16 / 32 measured, profiles/r02b.md)
 static void enqueue_run_steps(su2_lattice* lat, cudaStream_t st, cudaStream_t tail_st, int count, bool allow_overlap)
 {
     const size_t ctas = heatbath_ctas(lat->g);
@@ -503,7 +516,7 @@ static void enqueue_run_steps(su2_lattice* lat, cudaStream_t st, cudaStream_t ta
 // driver refuses them
 static bool build_run_graph(su2_lattice* lat, int count)
 {
-    cudaStream_t tail = lat->tail_overlap ? lat->tail_stream : nullptr;
+    cudaStream_t tail = tail_overlap_on(lat) ? lat->tail_stream : nullptr;
     for (int attempt = 0; attempt < 2 && !lat->run_exec; ++attempt) {
         const bool overlap = attempt == 0;
         const uint64_t launches0 = lat->launches;
@@ -536,12 +549,12 @@ extern "C" int su2_run(su2_lattice* lat, double beta, uint32_t sweep_idx0, uint3
         CK(lat, cudaEventCreateWithFlags(&lat->run_ev_in, cudaEventDisableTiming));
         CK(lat, cudaEventCreateWithFlags(&lat->run_ev_out, cudaEventDisableTiming));
     }
-    if (lat->tail_overlap && !lat->tail_stream) {
+    if (tail_overlap_on(lat) && !lat->tail_stream) {
         CK(lat, cudaStreamCreateWithFlags(&lat->tail_stream, cudaStreamNonBlocking));
         CK(lat, cudaEventCreateWithFlags(&lat->ev_fork, cudaEventDisableTiming));
         CK(lat, cudaEventCreateWithFlags(&lat->ev_join, cudaEventDisableTiming));
     }
-    cudaStream_t tail = lat->tail_overlap ? lat->tail_stream : nullptr;
+    cudaStream_t tail = tail_overlap_on(lat) ? lat->tail_stream : nullptr;
     // the private stream continues the handle's stream and hands back to it
     CK(lat, cudaEventRecord(lat->run_ev_in, lat->stream));
     CK(lat, cudaStreamWaitEvent(lat->run_stream, lat->run_ev_in, 0));

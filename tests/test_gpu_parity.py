@@ -516,14 +516,17 @@ def test_run_follows_set_draw_and_bad_method_is_rejected(pkg):
     a.close(); b.close()
 
 
+@pytest.mark.parametrize("overlap", [0, None])
 @pytest.mark.parametrize("how", ["set_seed", "init"])
-def test_run_after_reseed_uses_the_new_seed(pkg, how):
+def test_run_after_reseed_uses_the_new_seed(pkg, how, overlap):
     """The captured step of su2_run carries the seed's expanded Philox keys as kernel parameters:
     a reseed (su2_set_seed, or su2_init with another seed) must drop it. run(seed A); reseed B;
     run must equal the step-by-step calls with seed B, bit for bit."""
     import torch
-    dims, prec, beta, n = (16, 8, 8, 4), 64, 2.3, 3
+    dims, prec, beta, n = (16, 8, 8, 4), 64, 2.3, 20   # 20 steps: a captured block of 16 (or 20 one-step graphs) + 4
     a, b = pkg.Lattice(dims, prec), pkg.Lattice(dims, prec)
+    if overlap is not None:
+        a.set_option("tail_overlap", overlap)   # None: the automatic default (on at this size)
     oa = torch.zeros(4 * n, dtype=torch.float64, device="cuda")
     ob = torch.zeros(4 * n, dtype=torch.float64, device="cuda")
     a.init("hot", 1)
@@ -543,12 +546,13 @@ def test_run_after_reseed_uses_the_new_seed(pkg, how):
     torch.cuda.synchronize()
     assert (a.get_links() == b.get_links()).all()
     assert torch.equal(oa, ob)
-    # ... and the oracle agrees on which stream that is
+    # ... and the oracle agrees on which stream that is: the first steps after the reseed (later ones drift apart
+    # chaotically from rounding, see test_config1_ten_sweeps_links_and_plaquette)
     if how == "init":
         L = oracle.init(dims, "hot", 2, "f64")
-        for i in range(n):
+        for i in range(3):
             oracle.heatbath_sweep(dims, L, beta, 2, n + i, "f64")
-        assert_links_equal_within_tol(a.get_links(), L, 64)
+            assert abs(float(oa[2 * (n + i)]) - oracle.mean_plaquette(dims, L, "f64")) < 1e-12
     a.close(); b.close()
 
 
@@ -557,11 +561,11 @@ def test_run_after_reseed_uses_the_new_seed(pkg, how):
 @pytest.mark.parametrize("dims", [(16, 8, 8, 4), (32, 32, 32, 32), (6, 4, 10, 2)])
 def test_run_with_tail_overlap_equals_plain_run_bitwise(pkg, dims, prec, graphs):
     """SU2_OPT_TAIL_OVERLAP: the Polyakov kernel of step i on a second stream beside step i+1, two alternating sets
-    of fused-plaquette partials and loop states, blocks of 8 steps per graph plus a directly enqueued remainder
-    (19 = 2 blocks + 3; 5 = remainder only). Links and every observable equal the plain su2_run's bit for bit."""
+    of fused-plaquette partials and loop states, blocks of 16 steps per graph plus a directly enqueued remainder. Links and every observable equal the plain su2_run's bit for bit."""
     import torch
-    n1, n2 = 19, 5
+    n1, n2 = 37, 5   # 37 = 2 blocks of 16 + 5 directly enqueued steps; 5 = remainder only
     a, b = pkg.Lattice(dims, prec), pkg.Lattice(dims, prec)
+    a.set_option("tail_overlap", 0)   # the plain run (the default is automatic: on for lattices of this size)
     b.set_option("tail_overlap", 1)
     b.set_option("run_graph", graphs)
     oa = torch.zeros(2 * (n1 + n2), dtype=torch.float64, device="cuda")
@@ -575,6 +579,7 @@ def test_run_with_tail_overlap_equals_plain_run_bitwise(pkg, dims, prec, graphs)
     assert (a.get_links() == b.get_links()).all()
     # switching the option off again drops the captured block
     b.set_option("tail_overlap", 0)
+    a.set_option("tail_overlap", 1)
     a.run(2.4, 100, 3, oa)
     b.run(2.4, 100, 3, ob)
     torch.cuda.synchronize()
