@@ -319,6 +319,14 @@ def time_aux(pkg, torch, workloads):
         dt = time.perf_counter() - t0
         out[f"C2_16^3x4_batch{R}"] = {"us_per_round": dt / n * 1e6, "value": R * w.links * n / dt, "unit": UNIT,
                                       "replicas": R, "precision": 32, "rounds": n}
+        # the same rounds as ONE su2_batch_run call (one round captured as a CUDA graph, replayed)
+        bat.batch_run(betas, 1000, 10, obs)
+        bat.synchronize()
+        t0 = time.perf_counter()
+        bat.batch_run(betas, 1010, n, obs)
+        bat.synchronize()
+        dt = time.perf_counter() - t0
+        out[f"C2_16^3x4_batch{R}"].update({"batch_run_us_per_round": dt / n * 1e6, "batch_run_value": R * w.links * n / dt})
         bat.close()
     # ... and the paper's benchmark shape: four 32^4 lattices stepped by the launches of one (a 32^4 launch is 3.5 CTA
     # waves and latency-bound; four of them are 14 waves)

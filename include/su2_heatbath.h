@@ -214,6 +214,14 @@ SU2_API int su2_batch_init(su2_lattice* lat, int start, const uint64_t* seeds);
  * initialised), SU2_ECUDA. */
 SU2_API int su2_batch_sweep_measure(su2_lattice* lat, const double* betas, uint32_t sweep_idx, double* dev_out,
                                     size_t index);
+/* su2_run for a batch: n_steps rounds of su2_batch_sweep_measure(betas, sweep_idx0 + i, dev_out, i) as one call - the
+ * beta scan of PAPER.md:63-72 as the paper's loop. One round (9 launches) is captured once per handle as a
+ * CUDA graph and replayed; the sweep index and the output slot live in device memory, couplings and seeds in the
+ * per-replica device table. dev_out [device] holds 2 * n_replicas * n_steps doubles: step i of replica r at
+ * dev_out[2*(i*n_replicas + r)] (plaquette) and + 1 (Polyakov loop). Same links and observables as the round-by-round
+ * calls, bit for bit. Runs on the private stream of su2_run, ordered after and joined back into the handle's stream.
+ * Asynchronous (a change of betas or seeds first waits for the stream). Errors as su2_batch_sweep_measure. */
+SU2_API int su2_batch_run(su2_lattice* lat, const double* betas, uint32_t sweep_idx0, uint32_t n_steps, double* dev_out);
 
 /* NEXT-1 (eq. 3): on-axis Polyakov-loop correlator
  * C(r) = < l(x) l(x + r e_i) >, averaged over all spatial x and the 3 spatial axes i,

@@ -39,6 +39,7 @@ _SIGNATURES = {
     "su2_select_replica": (C.c_int, [C.c_void_p, C.c_int]),
     "su2_batch_init": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
     "su2_batch_sweep_measure": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_size_t]),
+    "su2_batch_run": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p]),
     "su2_lattice_destroy": (C.c_int, [C.c_void_p]),
     "su2_set_stream": (C.c_int, [C.c_void_p, C.c_void_p]),
     "su2_init": (C.c_int, [C.c_void_p, C.c_int, C.c_uint64]),
@@ -158,6 +159,11 @@ def su2_batch_init(h, start, seeds):
 def su2_batch_sweep_measure(h, betas, sweep_idx, dev_out_ptr, index):
     a = np.ascontiguousarray(betas, dtype=np.float64)
     _check(lib().su2_batch_sweep_measure(h, C.c_void_p(a.ctypes.data), sweep_idx, C.c_void_p(dev_out_ptr), index), h)
+
+
+def su2_batch_run(h, betas, sweep_idx0, n_steps, dev_out_ptr):
+    a = np.ascontiguousarray(betas, dtype=np.float64)
+    _check(lib().su2_batch_run(h, C.c_void_p(a.ctypes.data), sweep_idx0, n_steps, C.c_void_p(dev_out_ptr)), h)
 
 
 def su2_lattice_destroy(h):
@@ -376,6 +382,11 @@ class Lattice:
         """dev_out: float64 device tensor; step `index` of replica r lands at [2*(index*replicas + r) + {0,1}]."""
         assert len(betas) == self.replicas and dev_out.numel() >= 2 * self.replicas * (index + 1)
         su2_batch_sweep_measure(self.h, betas, sweep_idx, dev_out.data_ptr(), index)
+
+    def batch_run(self, betas, sweep_idx0, n_steps, dev_out):
+        """n_steps rounds as one call; step i of replica r lands at dev_out[2*(i*replicas + r) + {0,1}]."""
+        assert len(betas) == self.replicas and dev_out.numel() >= 2 * self.replicas * n_steps
+        su2_batch_run(self.h, betas, sweep_idx0, n_steps, dev_out.data_ptr())
 
     def set_draw(self, method):
         su2_set_draw(self.h, {"kp": SU2_DRAW_KP, "auto": SU2_DRAW_AUTO, "creutz": SU2_DRAW_CREUTZ}[method])

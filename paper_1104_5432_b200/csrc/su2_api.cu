@@ -29,6 +29,7 @@ struct su2_lattice {
     cudaStream_t run_stream;
     cudaEvent_t run_ev_in, run_ev_out;
     cudaGraphExec_t run_exec;
+    cudaGraphExec_t batch_exec;  // su2_batch_run: one round of the whole batch
     bool run_graphs;   // su2_run replays a captured CUDA graph (su2_set_option SU2_OPT_RUN_GRAPH)
     int tail_overlap;  // su2_run: the Polyakov kernel of a step runs beside the next step (SU2_OPT_TAIL_OVERLAP):
                        // 0 off, 1 on, -1 (default) automatic - see tail_overlap_on()
@@ -182,8 +183,8 @@ static int create_impl(int Nx, int Ny, int Nz, int Nt, int precision, int nrep, 
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.out, (2 + kMaxR) * sizeof(double));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.state, 2 * kRunCopies * sizeof(RunState));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.slots, (size_t)nrep * 2 * (v3 / 64 + 1) * sizeof(double));
-    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.ticket, (size_t)nrep * sizeof(unsigned));
-    if (ce == cudaSuccess) ce = cudaMemset(lat->sc.ticket, 0, (size_t)nrep * sizeof(unsigned));
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.ticket, ((size_t)nrep + 1) * sizeof(unsigned));
+    if (ce == cudaSuccess) ce = cudaMemset(lat->sc.ticket, 0, ((size_t)nrep + 1) * sizeof(unsigned));
     if (ce == cudaSuccess) ce = cudaMalloc((void**)&lat->sc.err, sizeof(int));
     if (ce == cudaSuccess) ce = cudaMemset(lat->sc.err, 0, sizeof(int));
     if (ce != cudaSuccess) {
@@ -238,6 +239,7 @@ extern "C" int su2_lattice_destroy(su2_lattice* lat)
     if (lat->sc.slots) cudaFree(lat->sc.slots);
     if (lat->sc.ticket) cudaFree(lat->sc.ticket);
     if (lat->run_exec) cudaGraphExecDestroy(lat->run_exec);
+    if (lat->batch_exec) cudaGraphExecDestroy(lat->batch_exec);
     if (lat->run_ev_in) cudaEventDestroy(lat->run_ev_in);
     if (lat->run_ev_out) cudaEventDestroy(lat->run_ev_out);
     if (lat->run_stream) cudaStreamDestroy(lat->run_stream);
@@ -264,6 +266,11 @@ static void drop_run_graph(su2_lattice* lat)
         cudaStreamSynchronize(lat->run_stream);
         cudaGraphExecDestroy(lat->run_exec);
         lat->run_exec = nullptr;
+    }
+    if (lat->batch_exec) {  // (seeds and couplings of a batch live in device memory: only the kernels are captured)
+        cudaStreamSynchronize(lat->run_stream);
+        cudaGraphExecDestroy(lat->batch_exec);
+        lat->batch_exec = nullptr;
     }
 }
 
@@ -382,6 +389,86 @@ extern "C" int su2_batch_sweep_measure(su2_lattice* lat, const double* betas, ui
                                           dev_out + 2 * index * (size_t)lat->nrep, nullptr, lat->pdl, lat->stream,
                                           lat->nrep);
     CK(lat, cudaGetLastError());
+    return SU2_OK;
+}
+
+// one round of the whole batch on stream `st`, sweep index and output slot read from the device RunState
+static void enqueue_batch_round(su2_lattice* lat, cudaStream_t st, bool allow_overlap)
+{
+    const size_t ctas = heatbath_ctas(lat->g);
+    int prev = -1;
+    for (int mu = 0; mu < 4; ++mu)
+        for (int p = 0; p < 2; ++p) {
+            const int idx = 2 * mu + p;
+            const bool overlap = allow_overlap && lat->pdl && prev == (idx + 7) % 8;
+            lat->launches += launch_heatbath_substep(
+                lat->links_base, lat->g, lat->precision, mu, p, 1.0, lat->creutz_below, 0, 0u, lat->sc.err,
+                (p == 1 && mu >= 1) ? lat->sc.epart + (mu - 1) * ctas : nullptr, lat->sc.state, overlap, st, lat->sc.reps,
+                lat->nrep);
+            prev = idx;
+        }
+    lat->launches += launch_polyakov_step(lat->links_base, lat->g, lat->precision, lat->sc, lat->sc.epart, 3 * ctas,
+                                          1.0 / (6.0 * 2.0 * (double)lat->g.vh), nullptr, lat->sc.state,
+                                          allow_overlap && lat->pdl, st, lat->nrep);
+}
+
+// su2_run's counterpart for a batch: n rounds of su2_batch_sweep_measure as one call; one round is
+// captured as a CUDA graph and replayed, sweep index and output slot live in the device loop state.
+extern "C" int su2_batch_run(su2_lattice* lat, const double* betas, uint32_t sweep_idx0, uint32_t n_steps, double* dev_out)
+{
+    ENTER(lat);
+    NOT_ON_A_SLAB(lat, "su2_batch_run");
+    NOT_A_SUBSTEP(lat);
+    if (!betas || (!dev_out && n_steps)) return fail(lat, SU2_EARG, "su2_batch_run: NULL argument");
+    bool changed = false;
+    for (int r = 0; r < lat->nrep; ++r) {
+        if (!(betas[r] > 0.0) || !isfinite(betas[r])) return fail(lat, SU2_EARG, "beta must be finite and > 0");
+        if (!lat->rep_init[r]) return fail(lat, SU2_ESTATE, "a replica of the batch is not initialised");
+        const RepParams rp = {1.0 / betas[r], lat->rep_seed[r]};
+        changed = changed || rp.inv_beta != lat->rep_host[r].inv_beta || rp.seed != lat->rep_host[r].seed;
+        lat->rep_host[r] = rp;
+    }
+    if (n_steps == 0) return SU2_OK;
+    if (changed) {  // rare: the kernels of earlier steps must have read the old values first
+        CK(lat, cudaStreamSynchronize(lat->stream));
+        CK(lat, cudaMemcpyAsync(lat->sc.reps, lat->rep_host, (size_t)lat->nrep * sizeof(RepParams),
+                                cudaMemcpyHostToDevice, lat->stream));
+    }
+    if (!lat->run_stream) {
+        CK(lat, cudaStreamCreateWithFlags(&lat->run_stream, cudaStreamNonBlocking));
+        CK(lat, cudaEventCreateWithFlags(&lat->run_ev_in, cudaEventDisableTiming));
+        CK(lat, cudaEventCreateWithFlags(&lat->run_ev_out, cudaEventDisableTiming));
+    }
+    CK(lat, cudaEventRecord(lat->run_ev_in, lat->stream));
+    CK(lat, cudaStreamWaitEvent(lat->run_stream, lat->run_ev_in, 0));
+    lat->launches += launch_set_run_state(lat->sc.state, 1.0, dev_out, sweep_idx0, 0u, lat->run_stream);
+    if (lat->run_graphs && !lat->batch_exec) {
+        for (int attempt = 0; attempt < 2 && !lat->batch_exec; ++attempt) {
+            const uint64_t launches0 = lat->launches;
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(lat->run_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) break;
+            enqueue_batch_round(lat, lat->run_stream, attempt == 0);
+            cudaError_t ce = cudaStreamEndCapture(lat->run_stream, &graph);
+            lat->launches = launches0;  // captured, not launched
+            if (ce == cudaSuccess && graph) ce = cudaGraphInstantiate(&lat->batch_exec, graph, 0);
+            if (graph) cudaGraphDestroy(graph);
+            if (ce != cudaSuccess) {
+                lat->batch_exec = nullptr;
+                cudaGetLastError();
+            }
+        }
+    }
+    for (uint32_t i = 0; i < n_steps; ++i) {
+        if (lat->run_graphs && lat->batch_exec) {
+            CK(lat, cudaGraphLaunch(lat->batch_exec, lat->run_stream));
+            lat->launches += 9;
+        } else {
+            enqueue_batch_round(lat, lat->run_stream, true);
+        }
+    }
+    CK(lat, cudaGetLastError());
+    CK(lat, cudaEventRecord(lat->run_ev_out, lat->run_stream));
+    CK(lat, cudaStreamWaitEvent(lat->stream, lat->run_ev_out, 0));
     return SU2_OK;
 }
 

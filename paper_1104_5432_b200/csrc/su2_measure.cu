@@ -143,7 +143,7 @@ struct StepTail {
     size_t n_epart;
     double scale_plaq, scale_poly;
     double* slots;        // [device] 2 * gridDim.x doubles per replica
-    unsigned* ticket;     // [device] one per replica, zero between steps
+    unsigned* ticket;     // [device] one per replica + one for the whole batch, zero between steps
     double* dst;          // [device] 2 doubles per replica (ignored when state != NULL)
     RunState* state;      // su2_run: destination state->out[2*index..], then sweep and index advance
     unsigned advance;     // ... by this much (1; 2 when two loop states alternate)
@@ -176,11 +176,22 @@ __device__ __forceinline__ void step_tail(const StepTail& tl, double poly_tot, d
     }
     const double ta = block_sum(sa, red);
     const double tb = block_sum(sb, red);
+    const unsigned R = gridDim.y;  // replicas of a batched launch (1 otherwise)
     if (threadIdx.x == 0) {
-        double* dst = tl.state ? tl.state->out + 2 * (size_t)tl.state->index : tl.dst + 2 * (size_t)rep;
+        double* dst = tl.state ? tl.state->out + 2 * ((size_t)tl.state->index * R + rep) : tl.dst + 2 * (size_t)rep;
         dst[0] = ta * tl.scale_plaq;
         dst[1] = tb * tl.scale_poly;
         *ticket = 0u;
+    }
+    if (tl.state && R > 1) {  // su2_batch_run: the state advances once per round, after the last replica has read it
+        __shared__ bool all_done;
+        if (threadIdx.x == 0) {
+            __threadfence();
+            all_done = atomicAdd(tl.ticket + R, 1u) == R - 1;
+            if (all_done) tl.ticket[R] = 0u;
+        }
+        __syncthreads();
+        if (!all_done) return;
     }
     if (tl.state)  // su2_run: advance every copy of the loop state (this CTA is the last one running)
         for (int i = threadIdx.x; i < kRunCopies; i += blockDim.x) {

@@ -654,6 +654,57 @@ def test_batch_equals_single_lattices_bitwise_and_matches_oracle(pkg, oracle_dra
     bat.close()
 
 
+@pytest.mark.parametrize("graphs", [1, 0])
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("dims", [(16, 16, 16, 4), (32, 4, 4, 2), (6, 4, 10, 2)])
+def test_batch_run_equals_round_by_round_calls_bitwise(pkg, dims, prec, graphs):
+    """su2_batch_run (one round captured as a CUDA graph, replayed; sweep index and output slot in device memory, the
+    loop state advanced once per round by the last CTA of the last replica) against su2_batch_sweep_measure called
+    round by round: identical links of every replica and identical observables; two calls in a row, a change of
+    couplings in between, and - on the same handle - su2_run on one selected replica afterwards."""
+    import torch
+    R, n1, n2 = 5, 6, 5
+    seeds = [300 + r for r in range(R)]
+    b1 = [2.2 + 0.1 * r for r in range(R)]
+    b2 = [2.6 - 0.1 * r for r in range(R)]
+    a, b = pkg.Lattice(dims, prec, replicas=R), pkg.Lattice(dims, prec, replicas=R)
+    b.set_option("run_graph", graphs)
+    oa = torch.zeros(2 * R * (n1 + n2), dtype=torch.float64, device="cuda")
+    ob = torch.zeros(2 * R * (n1 + n2), dtype=torch.float64, device="cuda")
+    for lat in (a, b):
+        lat.batch_init("hot", seeds)
+    for i in range(n1):
+        a.batch_sweep_measure(b1, i, oa, i)
+    for i in range(n2):
+        a.batch_sweep_measure(b2, n1 + i, oa, n1 + i)
+    b.batch_run(b1, 0, n1, ob)
+    b.batch_run(b2, n1, n2, ob[2 * R * n1:])
+    torch.cuda.synchronize()
+    assert torch.equal(oa, ob)
+    assert float(oa.abs().min()) > 0.0          # every slot was written
+    for r in range(R):
+        a.select(r)
+        b.select(r)
+        assert (a.get_links() == b.get_links()).all(), r
+    # the single-lattice loop on a replica of the same handle still works (it shares the loop state with the batch loop)
+    o1, o2 = torch.zeros(6, dtype=torch.float64, device="cuda"), torch.zeros(6, dtype=torch.float64, device="cuda")
+    a.select(2)
+    b.select(2)
+    for i in range(3):
+        a.sweep_measure(2.4, 50 + i, o1, i)
+    b.run(2.4, 50, 3, o2)
+    torch.cuda.synchronize()
+    assert torch.equal(o1, o2) and (a.get_links() == b.get_links()).all()
+    b.batch_run(b1, 60, 2, ob)                 # ... and the batch loop after it
+    for i in range(2):
+        a.batch_sweep_measure(b1, 60 + i, oa, i)
+    torch.cuda.synchronize()
+    assert torch.equal(oa[:4 * R], ob[:4 * R])
+    with pytest.raises(pkg.SU2Error):
+        b.batch_run([2.3] * (R - 1) + [-1.0], 70, 1, ob)
+    a.close(); b.close()
+
+
 @pytest.mark.parametrize("dims,R,why", [
     ((32, 4, 64, 64), 40, "2048 z-t tiles of the first shape x 40 replicas exceed grid z: second tile shape"),
     ((16, 4, 64, 128), 33, "first shape does not divide Nx/2 = 8, second gives 2048 x 33 > 65535: linear launch"),
